@@ -13,8 +13,9 @@
 //   O7  observer at a fixed location, bilinear interpolation (reading A11).
 // T is double, MP<2> (double-double) or MP<4> (quad-double) from mpx.hpp.
 // A sub-window [i_lo, i_lo+n_win) of the radial grid can be stepped on its own (Dirichlet rows at
-// the window edges); by the domain of dependence (i-1..i+1 per step) its interior
-// [i_lo+k, i_lo+n_win-1-k] equals the full-grid result after k steps.  Full grid: i_lo=0, n_win=N_r.
+// the window edges, zeroed at set_initial); by the domain of dependence (i-1..i+1 per step) its
+// interior [i_lo+k+1, i_lo+n_win-2-k] equals the full-grid result after k steps.
+// Full grid: i_lo=0, n_win=N_r.
 #include <cmath>
 #include <cstdio>
 #include <vector>

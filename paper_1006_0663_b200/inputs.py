@@ -82,14 +82,35 @@ class Workload:
         return replace(self, **kw)
 
 
+def stable_dt(w: Workload, z_max: float = 0.2) -> float:
+    """Harness time-step rule (reading A15b).  The two-step scheme of Eqs. (13)-(14) advances an
+    undamped oscillator  Phi_tt = -omega^2 Phi  with amplification 1 + (omega dt)^4/8 per step, so the stiffest
+    angular mode near the peak of kappa = Delta/Sigma^2 (omega^2 ~ kappa_max [4/dtheta^2 + (|m|+|s|)^2 /
+    sin^2(dtheta/2)], the second term being the pole potential of (m + s cos)^2/sin^2) grows unless omega dt is
+    small.  Measured with the oracle: config 2 at dt = 0.5 dr* overflows within 1500 steps.  For (s, m) != (0, 0)
+    the harness therefore passes dt = min(0.5 dr*, z_max / omega_max); work per update is unchanged.
+    This is input generation only (fp64 estimate), not part of the method's arithmetic."""
+    half_dr = 0.5 * w.dr
+    if w.s == 0 and w.m == 0:
+        return half_dr
+    rp = w.M + math.sqrt(w.M * w.M - w.a * w.a)
+    r = rp + np.linspace(1e-3, 20.0, 20001)
+    delta = r * r - 2.0 * w.M * r + w.a * w.a
+    kappa_max = float(np.max(delta / (r * r + w.a * w.a) ** 2))
+    dth = math.pi / w.n_theta
+    om2 = kappa_max * (4.0 / dth ** 2 + (abs(w.m) + abs(w.s)) ** 2 / math.sin(0.5 * dth) ** 2)
+    return min(half_dr, z_max / math.sqrt(om2))
+
+
 def config(k: int) -> Workload:
     """BASELINE.json configs 1..4 (SURVEY §8(d) 'Concrete inputs')."""
     if k == 1:
         return Workload("cfg1", 1.0, 0.0, 0, 0, 512, 16, -50.0, 150.0, 2000, 1, "P2",
                         (20.0, 2.0), (4.0, 0.5), (1.0, 0.1), SEED_BASE + 1, 40.0, 0.5 * math.pi)
     if k == 2:
-        return Workload("cfg2", 1.0, 0.9, -2, 2, 16384, 64, -300.0, 700.0, 20000, 1, "Y22m2",
-                        (100.0, 5.0), (6.0, 1.0), (1.0, 0.0), SEED_BASE + 2)
+        w = Workload("cfg2", 1.0, 0.9, -2, 2, 16384, 64, -300.0, 700.0, 20000, 1, "Y22m2",
+                     (100.0, 5.0), (6.0, 1.0), (1.0, 0.0), SEED_BASE + 2)
+        return replace(w, dt_override=stable_dt(w))
     if k == 3:
         return replace(config(2), name="cfg3", precision=2)   # same seed as cfg 2 ("same doubles")
     if k == 4:
@@ -99,20 +120,11 @@ def config(k: int) -> Workload:
 
 
 def sweep_cell(n_r: int, n_theta: int, precision: int) -> Workload:
-    """BASELINE.json config 5: a = 0.99, s = -2, m = 2, r* in [-300, 700] (A15), 1000 steps.
-
-    dt = 0.5 dr* where the explicit scheme is stable, else the reduced dt of
-    SURVEY §8(d) 'Stability caveat' (a harness choice; work per update is unchanged)."""
+    """BASELINE.json config 5: a = 0.99, s = -2, m = 2, r* in [-300, 700] (A15), 1000 steps,
+    dt from `stable_dt` (z_max = 0.4: 1000 steps tolerate a larger per-step growth)."""
     w = Workload(f"cfg5_{n_r}x{n_theta}_L{precision}", 1.0, 0.99, -2, 2, n_r, n_theta, -300.0, 700.0,
                  1000, precision, "Y22m2", (100.0, 5.0), (6.0, 1.0), (1.0, 0.0), SEED_BASE + 5)
-    dr = w.dr
-    dth = math.pi / n_theta
-    kappa_max = 0.0446                       # max Delta/Sigma^2 for a = 0.99 (SURVEY §8(d))
-    w_pole = kappa_max * 16.0 / math.sin(0.5 * dth) ** 2
-    dt_stable = 0.5 / math.sqrt(1.0 / dr ** 2 + kappa_max / dth ** 2 + w_pole / 4.0)
-    if dt_stable < 0.5 * dr:
-        w = replace(w, dt_override=dt_stable)
-    return w
+    return replace(w, dt_override=stable_dt(w, z_max=0.4))
 
 
 def theta_profile(profile: str, n_theta: int) -> np.ndarray:
@@ -121,7 +133,10 @@ def theta_profile(profile: str, n_theta: int) -> np.ndarray:
     if profile == "P0":
         return np.ones(n_theta)
     if profile == "P2":
-        return 0.5 * (3.0 * c * c - 1.0)
+        y = 0.5 * (3.0 * c * c - 1.0)
+        half = n_theta // 2                  # mirrored so the data are exactly theta -> pi - theta symmetric
+        y[n_theta - half:] = y[:half][::-1]
+        return y
     if profile == "Y22m2":                   # _{-2}Y_{22}(theta) real profile
         return math.sqrt(5.0 / (64.0 * math.pi)) * (1.0 + c) ** 2
     raise ValueError(profile)
