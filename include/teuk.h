@@ -1,0 +1,98 @@
+/* teuk.h — C ABI of libteuk.so: the time step of the m-mode-reduced 2+1D Teukolsky equation as a
+ * first-order complex (Phi, Pi) system on an (r*, theta) grid in Kerr background, §III.B
+ * (PAPER.md:53-112), at three precisions: fp64, double-double, quad-double.
+ * Every step of the path runs in CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *  - All scalar parameters are fp64 and taken as exact.  Grid: r*_i = rstar_min + i dr*,
+ *    dr* = (rstar_max - rstar_min)/(n_r - 1), i = 0..n_r-1; theta_j = (j + 1/2) pi/n_theta.
+ *  - State planes: double[4][L][n_theta][n_r], i fastest; fields in the order of Eq. (9)
+ *    (PAPER.md:88): Phi_R, Phi_I, Pi_R, Pi_I; L = limbs per real (1, 2, 4), limb 0 leading.
+ *  - Every function returns a status code (TEUK_OK = 0, negative on error); out-parameters are
+ *    untouched on error.  One handle = one CUDA stream; handles are not thread-safe.
+ *  - Pointers named host_* are HOST memory owned by the caller; d_workspace is DEVICE memory owned
+ *    by the caller (e.g. a torch tensor) that must outlive the handle; cuda_stream is a borrowed
+ *    cudaStream_t (NULL = the legacy default stream).
+ */
+#ifndef TEUK_H
+#define TEUK_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct teuk_ctx teuk_ctx;
+
+enum { TEUK_FP64 = 1, TEUK_DD = 2, TEUK_QD = 4 };      /* value == limbs per real */
+enum { TEUK_OK = 0, TEUK_EINVAL = -1, TEUK_ENOMEM = -2, TEUK_ECUDA = -3, TEUK_ESTATE = -4, TEUK_ENONFINITE = -5 };
+
+/* Bytes of device workspace teuk_create needs (two state buffers, 16 L coefficient planes, 1-D
+ * tables, observer buffer for obs_capacity samples).  TEUK_EINVAL on bad sizes. */
+int teuk_workspace_bytes(int n_r, int n_theta, int precision, long obs_capacity, size_t *bytes);
+
+/* Build the time-independent tables on the device (r(r*) from Eq. (2); b from Eqs. (6)-(7)
+ * PAPER.md:76-80; alpha, gamma, W, kappa of S in Eq. (12) PAPER.md:98 derived from Eq. (1), see
+ * DESIGN.md §3), evaluated in quad-double and rounded to L limbs.  M > 0, |a| < M, n_r >= 3,
+ * n_theta >= 2, dt > 0, rstar_min < rstar_max, precision in {1, 2, 4}; else TEUK_EINVAL.
+ * obs_capacity = number of observer samples the workspace was sized for. */
+int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double rstar_min, double rstar_max,
+                double dt, int precision, void *d_workspace, size_t workspace_bytes, long obs_capacity,
+                void *cuda_stream, teuk_ctx **out);
+
+/* Options, only before teuk_set_initial (else TEUK_ESTATE): "graph_steps" (even, >= 2; steps per
+ * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic). */
+int teuk_set_option(teuk_ctx *, const char *key, double value);
+
+/* Observer at a fixed location: bilinear interpolation in (r*, theta) from the four
+ * surrounding nodes, weights fixed here.  Location must lie inside [r*_0, r*_{n_r-1}] x
+ * [theta_0, theta_{n_theta-1}], capacity <= obs_capacity of teuk_create; else TEUK_EINVAL.
+ * Resets the recorded series. */
+int teuk_set_observer(teuk_ctx *, double rstar_obs, double theta_obs, long capacity);
+
+/* Upload u^0: host_planes is double[4][limbs_in][n_theta][n_r], limbs_in in {1, L} (missing low limbs
+ * := 0).  Rows i = 0 and n_r-1 are forced to zero.  Resets step count and series. */
+int teuk_set_initial(teuk_ctx *, const double *host_planes, int limbs_in);
+/* Same with the planes already in DEVICE memory (no host traffic). */
+int teuk_set_initial_device(teuk_ctx *, const double *d_planes, int limbs_in);
+
+/* Advance n >= 0 iterations of Eqs. (13)-(14) with the radial and polar boundary
+ * conditions of PAPER.md:112 and one observer sample per iteration; asynchronous on the stream. */
+int teuk_step(teuk_ctx *, long n);
+
+/* Download the state, double[4][L][n_theta][n_r]; synchronises the stream. */
+int teuk_read(teuk_ctx *, double *host_planes);
+/* Copy the state into DEVICE memory of the same layout; asynchronous on the stream. */
+int teuk_read_device(teuk_ctx *, double *d_planes);
+
+/* Observer series: out[count][4][L] = Phi_R, Phi_I, Pi_R, Pi_I at the observer after each completed
+ * iteration (sample k <-> t = (k+1) dt), count <= max_samples; synchronises.  Returns
+ * TEUK_ENONFINITE (sticky, data still written) if any recorded sample was not finite. */
+int teuk_observe(teuk_ctx *, double *host_out, long max_samples, long *count);
+
+int teuk_steps_done(teuk_ctx *, long *n);
+/* Number of kernels this handle has launched so far (graph nodes counted per replay). */
+int teuk_launch_count(teuk_ctx *, long *n);
+/* Launch geometry of the step kernel: out[0..5] = tile_i, tile_j, threads, grid_x, grid_y, smem bytes. */
+int teuk_step_geometry(teuk_ctx *, long *out6);
+void teuk_destroy(teuk_ctx *);
+const char *teuk_strerror(int code);
+
+/* ---- test hooks (used by tests/ only) ------------------------------------------------------- */
+/* Coefficient planes as the kernel uses them, double[8][L][n_theta][rows] (rows = n_r, or n_r-1 when
+ * half != 0), UNFOLDED: b, alpha_R, alpha_I, gamma_R, gamma_I, W_R, W_I, kappa.  Host output. */
+int teuk_get_tables(teuk_ctx *, int half, double *host_out);
+/* r and r - r_+ at the 2 n_r - 1 integer/half points as quad-double limbs, double[2 n_r - 1][4] each. */
+int teuk_get_radial(teuk_ctx *, double *host_r, double *host_delta);
+/* One arithmetic operation of the multiprecision layer, limbs in/out (L = 2 or 4);
+ * op: 0 add, 1 sub, 2 mul, 3 div, 4 sqrt(a), 5 a * b[0];  on_device != 0 runs it in a kernel. */
+int teuk_test_mp_op(int op, int L, const double *a, const double *b, double *out, long n, int on_device);
+/* Quad-double elementary functions of the setup: fn 0 exp, 1 log, 2 sin, 3 cos, 4 pi, 5 ln2 (host build). */
+int teuk_test_mp_fn(int fn, const double *a, double *out);
+/* FP64-pipe microbenchmark: register-resident chains of DFMA (kind 0), DADD (1), DMUL (2);
+ * returns instructions per second over all SMs (used for the dd/qd roofline denominator). */
+int teuk_bench_fp64(int kind, long iters, double *inst_per_s, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,211 @@
+// Fused Lax-Wendroff step kernel: half step Eq. (13) + full step Eq. (14), radial
+// Dirichlet rows and polar parity ghosts and the observer node extraction
+// in ONE launch per iteration; the intermediate u^{n+1/2}_{i+1/2} lives only in shared
+// memory.  Templated on the limb count L (1 fp64, 2 double-double, 4 quad-double).
+//
+// Folded coefficient planes (built once by setup_coefficients, tau = dt/2 for the half step and dt
+// for the full step; everything a product of time-independent factors):
+//   c0 = tau b / dr*            c1,c2 = tau alpha / 2        c3,c4 = tau gamma / dr*
+//   c5,c6 = tau W / 2           c7 = tau kappa / (2 dtheta^2)
+// and the 1-D table cj[j] = cot(theta_j) dtheta / 2.  With sig = u_hi + u_lo, del = u_hi - u_lo
+// (the two radial neighbours) and Lam = ((sig+ + sig-) - 2 sig) + cj (sig+ - sig-) over theta:
+//   new_Phi = base_Phi - c0 del_Phi + (tau/2) sig_Pi
+//   new_Pi  = base_Pi  + c0 del_Pi  + [ -(c1 + i c2) sig_Pi + (c3 + i c4) del_Phi + c7 Lam - (c5 + i c6) sig_Phi ]
+// base = sig/2 for the half step, u^n for the full step.  Multiplications by 1/2 and 2 are exact.
+#pragma once
+#include "mp.cuh"
+
+namespace tk {
+
+struct StepParams {
+    const double* u_in;      // [4][L] planes of n_theta x pitch
+    double* u_out;
+    const double* coef_i;    // [8][L] planes, integer points (full step)
+    const double* coef_h;    // [8][L] planes, half points (column i <-> i + 1/2)
+    const double* cj;        // [L][n_theta]
+    int n_r, n_theta, pitch;
+    long plane;              // n_theta * pitch
+    int ti, tj;              // output tile
+    double sigma;            // +1 even |m|, -1 odd |m|
+    double tq_half, tq_full; // tau/2 = dt/4, dt/2
+    double* obs_raw;         // [cap][4 nodes][4][L] or null
+    const long* step_base;
+    long obs_cap;
+    int step_off;
+    int oi, oj;              // lower-left observer node
+};
+
+template <int L> struct Ld {
+    static __device__ __forceinline__ Real<L> g(const double* __restrict__ p, long stride, long idx) {
+        Real<L> r;
+#pragma unroll
+        for (int l = 0; l < L; ++l) r.x[l] = __ldg(p + l * stride + idx);
+        return r;
+    }
+    static __device__ __forceinline__ Real<L> s(const double* p, int stride, int idx) {
+        Real<L> r;
+#pragma unroll
+        for (int l = 0; l < L; ++l) r.x[l] = p[l * stride + idx];
+        return r;
+    }
+    static __device__ __forceinline__ void st(double* p, long stride, long idx, const Real<L>& v) {
+#pragma unroll
+        for (int l = 0; l < L; ++l) p[l * stride + idx] = v.x[l];
+    }
+};
+
+template <int L> __device__ __forceinline__ Real<L> sgn(const Real<L>& a, double s) {
+    Real<L> r;
+#pragma unroll
+    for (int l = 0; l < L; ++l) r.x[l] = a.x[l] * s;     // s = +-1: exact
+    return r;
+}
+
+// One sub-step at one point.  T: tile accessor giving Real<L> at (component, row offset, column).
+// lo/hi are the two radial neighbour columns in the tile; rows jm/jp are the theta neighbours
+// (already mirrored) with signs sm/sp.
+template <int L, class Tile>
+__device__ __forceinline__ void substep(const Tile& t, int row, int rm, int rp, double sm, double sp, int clo, int chi,
+                                        const double* __restrict__ coef, long cstride, long cidx, const Real<L>& cjv,
+                                        double tq, bool half, const Real<L> base_in[4], Real<L> out[4]) {
+    Real<L> sg[4], dl[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        Real<L> lo = t.get(c, row, clo), hi = t.get(c, row, chi);
+        sg[c] = add(hi, lo);
+        dl[c] = sub(hi, lo);
+    }
+    // angular operator on sig_Phi (components 0, 1)
+    Real<L> lam[2];
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        Real<L> up = sgn(add(t.get(c, rp, chi), t.get(c, rp, clo)), sp);
+        Real<L> dn = sgn(add(t.get(c, rm, chi), t.get(c, rm, clo)), sm);
+        Real<L> second = sub(add(up, dn), scale2(sg[c], 2.0));
+        Real<L> first = mul(cjv, sub(up, dn));
+        lam[c] = add(second, first);
+    }
+    Real<L> c0 = Ld<L>::g(coef + 0 * L * cstride, cstride, cidx);
+    Real<L> c1 = Ld<L>::g(coef + 1 * L * cstride, cstride, cidx);
+    Real<L> c2 = Ld<L>::g(coef + 2 * L * cstride, cstride, cidx);
+    Real<L> c3 = Ld<L>::g(coef + 3 * L * cstride, cstride, cidx);
+    Real<L> c4 = Ld<L>::g(coef + 4 * L * cstride, cstride, cidx);
+    Real<L> c5 = Ld<L>::g(coef + 5 * L * cstride, cstride, cidx);
+    Real<L> c6 = Ld<L>::g(coef + 6 * L * cstride, cstride, cidx);
+    Real<L> c7 = Ld<L>::g(coef + 7 * L * cstride, cstride, cidx);
+    // tau * S_Pi, summed in the printed order of S: -alpha Pi + gamma Phi_* + kappa Lam - W Phi
+    Real<L> sR = neg(sub(mul(c1, sg[2]), mul(c2, sg[3])));
+    Real<L> sI = neg(add(mul(c1, sg[3]), mul(c2, sg[2])));
+    sR = add(sR, sub(mul(c3, dl[0]), mul(c4, dl[1])));
+    sI = add(sI, add(mul(c3, dl[1]), mul(c4, dl[0])));
+    sR = add(sR, mul(c7, lam[0]));
+    sI = add(sI, mul(c7, lam[1]));
+    sR = sub(sR, sub(mul(c5, sg[0]), mul(c6, sg[1])));
+    sI = sub(sI, add(mul(c5, sg[1]), mul(c6, sg[0])));
+    Real<L> b0, b1, b2, b3;
+    if (half) {
+        b0 = scale2(sg[0], 0.5); b1 = scale2(sg[1], 0.5); b2 = scale2(sg[2], 0.5); b3 = scale2(sg[3], 0.5);
+    } else {
+        b0 = base_in[0]; b1 = base_in[1]; b2 = base_in[2]; b3 = base_in[3];
+    }
+    out[0] = add(sub(b0, mul(c0, dl[0])), mul_d(sg[2], tq));
+    out[1] = add(sub(b1, mul(c0, dl[1])), mul_d(sg[3], tq));
+    out[2] = add(add(b2, mul(c0, dl[2])), sR);
+    out[3] = add(add(b3, mul(c0, dl[3])), sI);
+}
+
+template <int L> struct SmemTile {
+    const double* p;
+    int rows, cols, row0;       // row0 = global row of tile row 0
+    __device__ __forceinline__ Real<L> get(int c, int grow, int col) const {
+        return Ld<L>::s(p + (c * L) * rows * cols, rows * cols, (grow - row0) * cols + col);
+    }
+};
+
+template <int L>
+__global__ void __launch_bounds__(256) step_kernel(StepParams P) {
+    extern __shared__ double smem[];
+    const int TI = P.ti, TJ = P.tj;
+    const int UC = TI + 2, UR = TJ + 4, HC = TI + 1, HR = TJ + 2;
+    double* us = smem;                       // [4L][UR][UC]
+    double* hs = smem + 4 * L * UR * UC;     // [4L][HR][HC]
+    const int i0 = blockIdx.x * TI, j0 = blockIdx.y * TJ;
+    const int iu0 = i0 - 1, ju0 = j0 - 2, jh0 = j0 - 1;
+    const int nt = P.n_theta, nr = P.n_r;
+    const int tid = threadIdx.x, nth = blockDim.x;
+
+    // ---- phase 0: stage the u^n tile (+1 column, +2 rows of halo); outside the grid -> 0
+    for (int idx = tid; idx < 4 * L * UR * UC; idx += nth) {
+        int tc = idx % UC, rest = idx / UC;
+        int tr = rest % UR, pl = rest / UR;
+        int gi = iu0 + tc, gj = ju0 + tr;
+        double v = 0.0;
+        if (gi >= 0 && gi < nr && gj >= 0 && gj < nt) v = __ldg(P.u_in + pl * P.plane + (long)gj * P.pitch + gi);
+        us[idx] = v;
+    }
+    __syncthreads();
+
+    SmemTile<L> ut{us, UR, UC, ju0};
+    // ---- phase 1: half step, Eq. (13), at (ih + 1/2, jh) for the columns/rows the full step needs
+    for (int idx = tid; idx < HR * HC; idx += nth) {
+        int tc = idx % HC, tr = idx / HC;
+        int ih = iu0 + tc, jh = jh0 + tr;
+        if (ih < 0 || ih > nr - 2 || jh < 0 || jh >= nt) continue;
+        int rm = jh - 1, rp = jh + 1;
+        double sm = 1.0, sp = 1.0;
+        if (rm < 0) { rm = 0; sm = P.sigma; }
+        if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+        Real<L> cjv = Ld<L>::g(P.cj, nt, jh);
+        Real<L> out[4];
+        substep<L>(ut, jh, rm, rp, sm, sp, tc, tc + 1, P.coef_h, P.plane, (long)jh * P.pitch + ih, cjv, P.tq_half,
+                   true, out, out);
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int l = 0; l < L; ++l) hs[(c * L + l) * HR * HC + tr * HC + tc] = out[c].x[l];
+    }
+    __syncthreads();
+
+    SmemTile<L> ht{hs, HR, HC, jh0};
+    // ---- phase 2: full step, Eq. (14), + radial Dirichlet rows + observer nodes
+    for (int idx = tid; idx < TJ * TI; idx += nth) {
+        int tc = idx % TI, tr = idx / TI;
+        int i = i0 + tc, j = j0 + tr;
+        if (i >= nr || j >= nt) continue;
+        Real<L> out[4];
+        if (i == 0 || i == nr - 1) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) out[c] = from_double<L>(0.0);
+        } else {
+            int rm = j - 1, rp = j + 1;
+            double sm = 1.0, sp = 1.0;
+            if (rm < 0) { rm = 0; sm = P.sigma; }
+            if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+            Real<L> base[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) base[c] = ut.get(c, j, tc + 1);
+            Real<L> cjv = Ld<L>::g(P.cj, nt, j);
+            // h columns: tile col tc <-> i - 1/2, tc + 1 <-> i + 1/2
+            substep<L>(ht, j, rm, rp, sm, sp, tc, tc + 1, P.coef_i, P.plane, (long)j * P.pitch + i, cjv, P.tq_full,
+                       false, base, out);
+        }
+        long g = (long)j * P.pitch + i;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) Ld<L>::st(P.u_out + (long)c * L * P.plane, P.plane, g, out[c]);
+        if (P.obs_raw != nullptr) {
+            int di = i - P.oi, dj = j - P.oj;
+            if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
+                long k = *P.step_base + P.step_off;
+                if (k < P.obs_cap) {
+                    double* o = P.obs_raw + ((k * 4 + (dj * 2 + di)) * 4) * L;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+#pragma unroll
+                        for (int l = 0; l < L; ++l) o[c * L + l] = out[c].x[l];
+                }
+            }
+        }
+    }
+}
+
+}  // namespace tk

@@ -1,0 +1,639 @@
+// libteuk.so — C ABI of include/teuk.h.  Host logic only marshals arguments, lays out the caller's
+// device workspace and launches kernels; every step of the path (table setup, stepping, boundary and
+// polar conditions, observer extraction and interpolation) runs in CUDA kernels for sm_100a.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "../../include/teuk.h"
+#include "mp.cuh"
+#include "setup_kernels.cuh"
+#include "setup_math.cuh"
+#include "step_kernel.cuh"
+
+using namespace tk;
+
+#define CK(call)                                  \
+    do {                                          \
+        cudaError_t e_ = (call);                  \
+        if (e_ != cudaSuccess) return TEUK_ECUDA; \
+    } while (0)
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+    int pitch;
+    long plane;
+    size_t state_a, state_b, coef_i, coef_h, cj, r_tab, d_tab, sin_tab, cos_tab, obs_raw, obs_out, scalars, total;
+};
+
+static Layout make_layout(int n_r, int n_theta, int L, long cap) {
+    Layout y;
+    y.pitch = (int)align_up((size_t)n_r, 16);
+    y.plane = (long)y.pitch * n_theta;
+    size_t off = 0;
+    auto take = [&](size_t doubles) {
+        size_t o = off;
+        off = align_up(off + doubles * sizeof(double), 256);
+        return o;
+    };
+    y.state_a = take((size_t)4 * L * y.plane);
+    y.state_b = take((size_t)4 * L * y.plane);
+    y.coef_i = take((size_t)8 * L * y.plane);
+    y.coef_h = take((size_t)8 * L * y.plane);
+    y.cj = take((size_t)L * n_theta);
+    y.r_tab = take((size_t)4 * (2 * n_r - 1));
+    y.d_tab = take((size_t)4 * (2 * n_r - 1));
+    y.sin_tab = take((size_t)4 * n_theta);
+    y.cos_tab = take((size_t)4 * n_theta);
+    y.obs_raw = take((size_t)(cap > 0 ? cap : 1) * 16 * L);
+    y.obs_out = take((size_t)(cap > 0 ? cap : 1) * 4 * L);
+    y.scalars = take(8);
+    y.total = off;
+    return y;
+}
+
+struct teuk_ctx {
+    double M, a, rmin, rmax, dt;
+    int s, m, n_r, n_theta, L;
+    long cap_alloc;
+    char* ws;
+    Layout lay;
+    cudaStream_t stream;
+    SetupConsts C;
+    // options
+    int graph_steps = 32, opt_ti = 0, opt_tj = 0;
+    // geometry
+    int ti = 0, tj = 0, threads = 256;
+    dim3 grid;
+    size_t smem = 0;
+    // state
+    bool have_init = false;
+    int cur = 0;                       // which state buffer holds u^n
+    long steps_done = 0, launches = 0;
+    // observer
+    long obs_cap = 0;
+    int oi = 0, oj = 0;
+    R4 wr, wt;
+    bool nonfinite = false;
+    cudaGraphExec_t graph[2] = {nullptr, nullptr};
+
+    double* dptr(size_t off) const { return (double*)(ws + off); }
+    double* state(int which) const { return dptr(which ? lay.state_b : lay.state_a); }
+    long* step_base() const { return (long*)(ws + lay.scalars); }
+    int* flag() const { return (int*)(ws + lay.scalars + 16); }
+};
+
+// ------------------------------------------------------------------------------------ small kernels
+__global__ void advance_kernel(long* base, long k) { *base += k; }
+
+template <int L>
+__global__ void observer_combine_kernel(const double* __restrict__ raw, double* __restrict__ out, long count, R4 wr,
+                                        R4 wt, int* flag) {
+    // bilinear interpolation of the four recorded nodes in working precision (reading A11)
+    long k = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (k >= count * 4) return;
+    long smp = k / 4;
+    int c = (int)(k % 4);
+    Real<L> w_r = narrow<L>(wr), w_t = narrow<L>(wt), one = from_double<L>(1.0);
+    Real<L> u[4];
+#pragma unroll
+    for (int nd = 0; nd < 4; ++nd)
+#pragma unroll
+        for (int l = 0; l < L; ++l) u[nd].x[l] = raw[((smp * 4 + nd) * 4 + c) * L + l];
+    Real<L> lo = add(mul(sub(one, w_r), u[0]), mul(w_r, u[1]));
+    Real<L> hi = add(mul(sub(one, w_r), u[2]), mul(w_r, u[3]));
+    Real<L> v = add(mul(sub(one, w_t), lo), mul(w_t, hi));
+    bool bad = false;
+#pragma unroll
+    for (int l = 0; l < L; ++l) {
+        out[k * L + l] = v.x[l];
+        bad |= !isfinite(v.x[l]);
+    }
+    if (bad) atomicOr(flag, 1);
+}
+
+// set_initial on the device: copy limbs_in planes per field into L planes (missing limbs := 0), force the
+// radial boundary rows to zero, source layout [4][limbs_in][n_theta][n_r] (unpadded)
+__global__ void load_state_kernel(const double* __restrict__ src, double* __restrict__ dst, int n_r, int n_theta,
+                                  int pitch, long plane, int L, int limbs_in) {
+    long idx = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    long per = (long)n_theta * n_r;
+    if (idx >= 4 * L * per) return;
+    int i = (int)(idx % n_r);
+    long rest = idx / n_r;
+    int j = (int)(rest % n_theta);
+    int pl = (int)(rest / n_theta);
+    int f = pl / L, l = pl % L;
+    double v = 0.0;
+    if (l < limbs_in && i != 0 && i != n_r - 1) v = src[((long)(f * limbs_in + l) * n_theta + j) * n_r + i];
+    dst[pl * plane + (long)j * pitch + i] = v;
+}
+__global__ void store_state_kernel(const double* __restrict__ src, double* __restrict__ dst, int n_r, int n_theta,
+                                   int pitch, long plane, int planes) {
+    long idx = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    long per = (long)n_theta * n_r;
+    if (idx >= planes * per) return;
+    int i = (int)(idx % n_r);
+    long rest = idx / n_r;
+    int j = (int)(rest % n_theta);
+    int pl = (int)(rest / n_theta);
+    dst[idx] = src[pl * plane + (long)j * pitch + i];
+}
+
+// ------------------------------------------------------------------------------------ create
+static bool valid_sizes(int n_r, int n_theta, int precision, long cap) {
+    return n_r >= 3 && n_theta >= 2 && (precision == 1 || precision == 2 || precision == 4) && cap >= 0 &&
+           (long)n_r * n_theta < (1L << 31);
+}
+
+extern "C" int teuk_workspace_bytes(int n_r, int n_theta, int precision, long obs_capacity, size_t* bytes) {
+    if (!bytes || !valid_sizes(n_r, n_theta, precision, obs_capacity)) return TEUK_EINVAL;
+    *bytes = make_layout(n_r, n_theta, precision, obs_capacity).total;
+    return TEUK_OK;
+}
+
+template <int L>
+static int launch_coef(teuk_ctx* c, int half, int fold, double* out) {
+    int cols = half ? c->n_r - 1 : c->n_r;
+    dim3 grid((cols + 127) / 128, c->n_theta);
+    coef_kernel<L><<<grid, 128, 0, c->stream>>>(c->C, c->dptr(c->lay.r_tab), c->dptr(c->lay.d_tab),
+                                                c->dptr(c->lay.sin_tab), c->dptr(c->lay.cos_tab), half, fold, out);
+    c->launches++;
+    return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+}
+static int launch_coef_any(teuk_ctx* c, int half, int fold, double* out) {
+    if (c->L == 1) return launch_coef<1>(c, half, fold, out);
+    if (c->L == 2) return launch_coef<2>(c, half, fold, out);
+    return launch_coef<4>(c, half, fold, out);
+}
+
+extern "C" int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double rstar_min, double rstar_max,
+                           double dt, int precision, void* d_workspace, size_t workspace_bytes, long obs_capacity,
+                           void* cuda_stream, teuk_ctx** out) {
+    if (!out || !d_workspace || !valid_sizes(n_r, n_theta, precision, obs_capacity)) return TEUK_EINVAL;
+    if (!(M > 0) || !(std::fabs(a) < M) || !(dt > 0) || !(rstar_min < rstar_max)) return TEUK_EINVAL;
+    if (!std::isfinite(M) || !std::isfinite(a) || !std::isfinite(dt) || !std::isfinite(rstar_min) ||
+        !std::isfinite(rstar_max))
+        return TEUK_EINVAL;
+    Layout lay = make_layout(n_r, n_theta, precision, obs_capacity);
+    if (workspace_bytes < lay.total || ((size_t)d_workspace % 256) != 0) return TEUK_EINVAL;
+    teuk_ctx* c = new (std::nothrow) teuk_ctx();
+    if (!c) return TEUK_ENOMEM;
+    c->M = M; c->a = a; c->s = s; c->m = m; c->n_r = n_r; c->n_theta = n_theta; c->L = precision;
+    c->rmin = rstar_min; c->rmax = rstar_max; c->dt = dt; c->cap_alloc = obs_capacity;
+    c->ws = (char*)d_workspace; c->lay = lay; c->stream = (cudaStream_t)cuda_stream;
+
+    // ---- host scalars in quad-double
+    QConst qc = q_constants();
+    SetupConsts& C = c->C;
+    C.M = from_double<4>(M);
+    C.a = from_double<4>(a);
+    R4 root = msqrt(sub(mul(C.M, C.M), mul(C.a, C.a)));
+    C.rp = add(C.M, root);
+    R4 rm = sub(C.M, root);
+    C.rpm = scale2(root, 2.0);
+    C.cplus = div(mul(scale2(C.M, 2.0), C.rp), C.rpm);
+    C.cminus = div(mul(scale2(C.M, 2.0), rm), C.rpm);
+    C.rmin = from_double<4>(rstar_min);
+    C.dr = div(sub(from_double<4>(rstar_max), C.rmin), from_double<4>((double)(n_r - 1)));
+    C.dth = div(qc.pi, from_double<4>((double)n_theta));
+    C.ln2 = qc.ln2;
+    C.tau_f = from_double<4>(dt);
+    C.tau_h = scale2(C.tau_f, 0.5);
+    C.s = s; C.m = m; C.n_r = n_r; C.n_theta = n_theta; C.pitch = lay.pitch; C.plane = lay.plane;
+
+    // ---- theta tables on the host (N_theta/2 Taylor evaluations), mirrored so they are exactly symmetric
+    std::vector<double> sn(4 * n_theta), cs(4 * n_theta), cjv((size_t)precision * n_theta);
+    for (int j = 0; j < (n_theta + 1) / 2; ++j) {
+        R4 th = mul(C.dth, add(from_double<4>((double)j), from_double<4>(0.5)));
+        R4 sj, cj;
+        q_sincos(th, sj, cj);
+        int jm = n_theta - 1 - j;
+        if (jm == j) cj = from_double<4>(0.0);
+        R4 cot = div(cj, sj);
+        R4 cjq = scale2(mul(cot, C.dth), 0.5);            // cot(theta_j) dtheta / 2
+        for (int l = 0; l < 4; ++l) {
+            sn[4 * j + l] = sj.x[l];  cs[4 * j + l] = cj.x[l];
+            sn[4 * jm + l] = sj.x[l]; cs[4 * jm + l] = -cj.x[l];
+        }
+        for (int l = 0; l < precision; ++l) {
+            cjv[(size_t)l * n_theta + j] = cjq.x[l];
+            cjv[(size_t)l * n_theta + jm] = (jm == j) ? 0.0 : -cjq.x[l];
+        }
+    }
+    int rc = TEUK_OK;
+    auto fail = [&](int code) { delete c; return code; };
+    if (cudaMemsetAsync(c->ws, 0, lay.total, c->stream) != cudaSuccess) return fail(TEUK_ECUDA);
+    if (cudaMemcpyAsync(c->dptr(lay.sin_tab), sn.data(), sn.size() * 8, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(c->dptr(lay.cos_tab), cs.data(), cs.size() * 8, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(c->dptr(lay.cj), cjv.data(), cjv.size() * 8, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+        return fail(TEUK_ECUDA);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return fail(TEUK_ECUDA);   // host vectors go out of scope
+
+    // ---- r(r*) and the coefficient planes on the device
+    int npts = 2 * n_r - 1;
+    radial_kernel<<<(npts + 63) / 64, 64, 0, c->stream>>>(C, c->dptr(lay.r_tab), c->dptr(lay.d_tab));
+    c->launches++;
+    if (cudaGetLastError() != cudaSuccess) return fail(TEUK_ECUDA);
+    if ((rc = launch_coef_any(c, 0, 1, c->dptr(lay.coef_i))) != TEUK_OK) return fail(rc);
+    if ((rc = launch_coef_any(c, 1, 1, c->dptr(lay.coef_h))) != TEUK_OK) return fail(rc);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return fail(TEUK_ECUDA);
+    *out = c;
+    return TEUK_OK;
+}
+
+extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
+    if (!c || !key) return TEUK_EINVAL;
+    if (c->have_init) return TEUK_ESTATE;
+    int v = (int)value;
+    if (!strcmp(key, "graph_steps")) {
+        if (v < 0 || (v % 2) != 0 || v > 4096) return TEUK_EINVAL;
+        c->graph_steps = v;
+    } else if (!strcmp(key, "tile_i")) {
+        if (v < 0 || v > 256) return TEUK_EINVAL;
+        c->opt_ti = v;
+    } else if (!strcmp(key, "tile_j")) {
+        if (v < 0 || v > 256) return TEUK_EINVAL;
+        c->opt_tj = v;
+    } else if (!strcmp(key, "threads")) {
+        if (v < 32 || v > 256 || (v % 32) != 0) return TEUK_EINVAL;
+        c->threads = v;
+    } else {
+        return TEUK_EINVAL;
+    }
+    return TEUK_OK;
+}
+
+extern "C" int teuk_set_observer(teuk_ctx* c, double rstar_obs, double theta_obs, long capacity) {
+    if (!c || capacity < 0 || capacity > c->cap_alloc || !std::isfinite(rstar_obs) || !std::isfinite(theta_obs))
+        return TEUK_EINVAL;
+    R4 x = div(sub(from_double<4>(rstar_obs), c->C.rmin), c->C.dr);
+    R4 y = sub(div(from_double<4>(theta_obs), c->C.dth), from_double<4>(0.5));
+    int i0 = (int)std::floor(x.x[0]), j0 = (int)std::floor(y.x[0]);
+    if (x.x[0] < 0 || x.x[0] > c->n_r - 1 || y.x[0] < 0 || y.x[0] > c->n_theta - 1) return TEUK_EINVAL;
+    if (i0 > c->n_r - 2) i0 = c->n_r - 2;
+    if (j0 > c->n_theta - 2) j0 = c->n_theta - 2;
+    c->wr = sub(x, from_double<4>((double)i0));
+    c->wt = sub(y, from_double<4>((double)j0));
+    c->oi = i0; c->oj = j0; c->obs_cap = capacity;
+    c->nonfinite = false;
+    for (int p = 0; p < 2; ++p)
+        if (c->graph[p]) { cudaGraphExecDestroy(c->graph[p]); c->graph[p] = nullptr; }
+    CK(cudaMemsetAsync(c->step_base(), 0, 32, c->stream));
+    return TEUK_OK;
+}
+
+// ------------------------------------------------------------------------------------ stepping
+static size_t smem_bytes(int L, int ti, int tj) {
+    return (size_t)4 * L * ((size_t)(ti + 2) * (tj + 4) + (size_t)(ti + 1) * (tj + 2)) * sizeof(double);
+}
+
+static int choose_geometry(teuk_ctx* c) {
+    int ti = c->opt_ti, tj = c->opt_tj;
+    if (ti == 0) ti = (c->L == 4) ? 16 : 32;
+    if (tj == 0) {
+        // whole theta extent when it fits (no theta halo, no redundant half-step rows), else strips of 16
+        int full = c->n_theta;
+        tj = (smem_bytes(c->L, ti, full) <= 100 * 1024 && full <= 64) ? full : ((c->L == 4) ? 8 : 16);
+    }
+    if (tj > c->n_theta) tj = c->n_theta;
+    if (ti > c->n_r) ti = c->n_r;
+    size_t sm = smem_bytes(c->L, ti, tj);
+    if (sm > 227 * 1024) return TEUK_EINVAL;
+    c->ti = ti; c->tj = tj; c->smem = sm;
+    c->grid = dim3((c->n_r + ti - 1) / ti, (c->n_theta + tj - 1) / tj);
+    cudaError_t e = cudaSuccess;
+    if (c->L == 1) e = cudaFuncSetAttribute(step_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (c->L == 2) e = cudaFuncSetAttribute(step_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (c->L == 4) e = cudaFuncSetAttribute(step_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    return e == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+}
+
+static int launch_step(teuk_ctx* c, int from, int step_off) {
+    StepParams P;
+    P.u_in = c->state(from);
+    P.u_out = c->state(from ^ 1);
+    P.coef_i = c->dptr(c->lay.coef_i);
+    P.coef_h = c->dptr(c->lay.coef_h);
+    P.cj = c->dptr(c->lay.cj);
+    P.n_r = c->n_r; P.n_theta = c->n_theta; P.pitch = c->lay.pitch; P.plane = c->lay.plane;
+    P.ti = c->ti; P.tj = c->tj;
+    P.sigma = (std::abs(c->m) % 2 == 0) ? 1.0 : -1.0;
+    P.tq_half = 0.25 * c->dt;
+    P.tq_full = 0.5 * c->dt;
+    P.obs_raw = c->obs_cap > 0 ? c->dptr(c->lay.obs_raw) : nullptr;
+    P.step_base = c->step_base();
+    P.obs_cap = c->obs_cap;
+    P.step_off = step_off;
+    P.oi = c->oi; P.oj = c->oj;
+    if (c->L == 1) step_kernel<1><<<c->grid, c->threads, c->smem, c->stream>>>(P);
+    else if (c->L == 2) step_kernel<2><<<c->grid, c->threads, c->smem, c->stream>>>(P);
+    else step_kernel<4><<<c->grid, c->threads, c->smem, c->stream>>>(P);
+    return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+}
+
+static int upload_initial(teuk_ctx* c, const double* d_src, int limbs_in) {
+    long total = 4L * c->L * c->n_theta * c->n_r;
+    load_state_kernel<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(
+        d_src, c->state(0), c->n_r, c->n_theta, c->lay.pitch, c->lay.plane, c->L, limbs_in);
+    c->launches++;
+    if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
+    CK(cudaMemsetAsync(c->step_base(), 0, 32, c->stream));
+    c->cur = 0; c->steps_done = 0; c->nonfinite = false;
+    if (!c->have_init) {
+        int rc = choose_geometry(c);
+        if (rc != TEUK_OK) return rc;
+    }
+    c->have_init = true;
+    return TEUK_OK;
+}
+
+extern "C" int teuk_set_initial_device(teuk_ctx* c, const double* d_planes, int limbs_in) {
+    if (!c || !d_planes || (limbs_in != 1 && limbs_in != c->L)) return TEUK_EINVAL;
+    return upload_initial(c, d_planes, limbs_in);
+}
+
+extern "C" int teuk_set_initial(teuk_ctx* c, const double* host_planes, int limbs_in) {
+    if (!c || !host_planes || (limbs_in != 1 && limbs_in != c->L)) return TEUK_EINVAL;
+    // stage through the not-yet-used second state buffer (large enough: limbs_in <= L, unpadded <= padded)
+    size_t bytes = (size_t)4 * limbs_in * c->n_theta * c->n_r * sizeof(double);
+    CK(cudaMemcpyAsync(c->state(1), host_planes, bytes, cudaMemcpyHostToDevice, c->stream));
+    int rc = upload_initial(c, c->state(1), limbs_in);
+    if (rc != TEUK_OK) return rc;
+    CK(cudaStreamSynchronize(c->stream));     // the caller may free host_planes
+    return TEUK_OK;
+}
+
+static int build_graph(teuk_ctx* c, int parity) {
+    cudaGraph_t g;
+    CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    int from = parity, rc = TEUK_OK;
+    for (int k = 0; k < c->graph_steps && rc == TEUK_OK; ++k) {
+        rc = launch_step(c, from, k);
+        from ^= 1;
+    }
+    advance_kernel<<<1, 1, 0, c->stream>>>(c->step_base(), c->graph_steps);
+    cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+    if (rc != TEUK_OK || e != cudaSuccess) return TEUK_ECUDA;
+    e = cudaGraphInstantiate(&c->graph[parity], g, 0);
+    cudaGraphDestroy(g);
+    return e == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+}
+
+extern "C" int teuk_step(teuk_ctx* c, long n) {
+    if (!c || n < 0) return TEUK_EINVAL;
+    if (!c->have_init) return TEUK_ESTATE;
+    long left = n;
+    const int K = c->graph_steps;
+    while (K > 0 && left >= K) {
+        if (!c->graph[c->cur]) {
+            int rc = build_graph(c, c->cur);
+            if (rc != TEUK_OK) return rc;
+        }
+        CK(cudaGraphLaunch(c->graph[c->cur], c->stream));
+        c->launches += K + 1;
+        left -= K;                            // K is even: c->cur unchanged
+    }
+    if (left > 0) {
+        for (long k = 0; k < left; ++k) {
+            int rc = launch_step(c, c->cur, (int)k);
+            if (rc != TEUK_OK) return rc;
+            c->cur ^= 1;
+        }
+        advance_kernel<<<1, 1, 0, c->stream>>>(c->step_base(), left);
+        c->launches += left + 1;
+        if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
+    }
+    c->steps_done += n;
+    return TEUK_OK;
+}
+
+extern "C" int teuk_read_device(teuk_ctx* c, double* d_planes) {
+    if (!c || !d_planes) return TEUK_EINVAL;
+    if (!c->have_init) return TEUK_ESTATE;
+    long total = 4L * c->L * c->n_theta * c->n_r;
+    store_state_kernel<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(
+        c->state(c->cur), d_planes, c->n_r, c->n_theta, c->lay.pitch, c->lay.plane, 4 * c->L);
+    c->launches++;
+    return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+}
+
+extern "C" int teuk_read(teuk_ctx* c, double* host_planes) {
+    if (!c || !host_planes) return TEUK_EINVAL;
+    if (!c->have_init) return TEUK_ESTATE;
+    // unpad through the idle state buffer, then one D2H copy
+    double* tmp = c->state(c->cur ^ 1);
+    int rc = teuk_read_device(c, tmp);
+    if (rc != TEUK_OK) return rc;
+    size_t bytes = (size_t)4 * c->L * c->n_theta * c->n_r * sizeof(double);
+    CK(cudaMemcpyAsync(host_planes, tmp, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return TEUK_OK;
+}
+
+extern "C" int teuk_observe(teuk_ctx* c, double* host_out, long max_samples, long* count) {
+    if (!c || !host_out || !count || max_samples < 0) return TEUK_EINVAL;
+    long n = c->steps_done < c->obs_cap ? c->steps_done : c->obs_cap;
+    if (n > max_samples) n = max_samples;
+    if (n > 0) {
+        unsigned blocks = (unsigned)((n * 4 + 127) / 128);
+        const double* raw = c->dptr(c->lay.obs_raw);
+        double* out = c->dptr(c->lay.obs_out);
+        if (c->L == 1) observer_combine_kernel<1><<<blocks, 128, 0, c->stream>>>(raw, out, n, c->wr, c->wt, c->flag());
+        else if (c->L == 2) observer_combine_kernel<2><<<blocks, 128, 0, c->stream>>>(raw, out, n, c->wr, c->wt, c->flag());
+        else observer_combine_kernel<4><<<blocks, 128, 0, c->stream>>>(raw, out, n, c->wr, c->wt, c->flag());
+        c->launches++;
+        if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
+        CK(cudaMemcpyAsync(host_out, out, (size_t)n * 4 * c->L * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        int flag = 0;
+        CK(cudaMemcpyAsync(&flag, c->flag(), sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        if (flag) c->nonfinite = true;
+    } else {
+        CK(cudaStreamSynchronize(c->stream));
+    }
+    *count = n;
+    return c->nonfinite ? TEUK_ENONFINITE : TEUK_OK;
+}
+
+extern "C" int teuk_steps_done(teuk_ctx* c, long* n) {
+    if (!c || !n) return TEUK_EINVAL;
+    *n = c->steps_done;
+    return TEUK_OK;
+}
+extern "C" int teuk_launch_count(teuk_ctx* c, long* n) {
+    if (!c || !n) return TEUK_EINVAL;
+    *n = c->launches;
+    return TEUK_OK;
+}
+extern "C" int teuk_step_geometry(teuk_ctx* c, long* o) {
+    if (!c || !o) return TEUK_EINVAL;
+    if (!c->have_init) return TEUK_ESTATE;
+    o[0] = c->ti; o[1] = c->tj; o[2] = c->threads; o[3] = c->grid.x; o[4] = c->grid.y; o[5] = (long)c->smem;
+    return TEUK_OK;
+}
+extern "C" void teuk_destroy(teuk_ctx* c) {
+    if (!c) return;
+    for (int p = 0; p < 2; ++p)
+        if (c->graph[p]) cudaGraphExecDestroy(c->graph[p]);
+    delete c;
+}
+extern "C" const char* teuk_strerror(int code) {
+    switch (code) {
+        case TEUK_OK: return "ok";
+        case TEUK_EINVAL: return "invalid argument";
+        case TEUK_ENOMEM: return "out of memory";
+        case TEUK_ECUDA: return "CUDA error";
+        case TEUK_ESTATE: return "call not valid in this state";
+        case TEUK_ENONFINITE: return "non-finite observer sample";
+        default: return "unknown error";
+    }
+}
+
+// ------------------------------------------------------------------------------------ test hooks
+extern "C" int teuk_get_tables(teuk_ctx* c, int half, double* host_out) {
+    if (!c || !host_out) return TEUK_EINVAL;
+    int rows = half ? c->n_r - 1 : c->n_r;
+    size_t padded = (size_t)8 * c->L * c->lay.plane * sizeof(double);
+    double* tmp = nullptr;
+    if (cudaMalloc(&tmp, padded) != cudaSuccess) return TEUK_ENOMEM;
+    int rc = launch_coef_any(c, half ? 1 : 0, 0, tmp);
+    std::vector<double> h((size_t)8 * c->L * c->lay.plane);
+    if (rc == TEUK_OK && (cudaMemcpyAsync(h.data(), tmp, padded, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+                          cudaStreamSynchronize(c->stream) != cudaSuccess))
+        rc = TEUK_ECUDA;
+    cudaFree(tmp);
+    if (rc != TEUK_OK) return rc;
+    for (int pl = 0; pl < 8 * c->L; ++pl)
+        for (int j = 0; j < c->n_theta; ++j)
+            for (int i = 0; i < rows; ++i)
+                host_out[((size_t)pl * c->n_theta + j) * rows + i] = h[(size_t)pl * c->lay.plane + (size_t)j * c->lay.pitch + i];
+    return TEUK_OK;
+}
+
+extern "C" int teuk_get_radial(teuk_ctx* c, double* host_r, double* host_delta) {
+    if (!c || !host_r || !host_delta) return TEUK_EINVAL;
+    size_t bytes = (size_t)4 * (2 * c->n_r - 1) * sizeof(double);
+    CK(cudaMemcpyAsync(host_r, c->dptr(c->lay.r_tab), bytes, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaMemcpyAsync(host_delta, c->dptr(c->lay.d_tab), bytes, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return TEUK_OK;
+}
+
+template <int L> MPX Real<L> mp_apply(int op, const Real<L>& x, const Real<L>& y) {
+    switch (op) {
+        case 0: return add(x, y);
+        case 1: return sub(x, y);
+        case 2: return mul(x, y);
+        case 3: return div(x, y);
+        case 4: return msqrt(x);
+        default: return mul_d(x, y.x[0]);
+    }
+}
+template <int L> __global__ void mp_op_kernel(int op, const double* a, const double* b, double* out, long n) {
+    long k = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    Real<L> x, y;
+    for (int l = 0; l < L; ++l) { x.x[l] = a[k * L + l]; y.x[l] = b[k * L + l]; }
+    Real<L> r = mp_apply<L>(op, x, y);
+    for (int l = 0; l < L; ++l) out[k * L + l] = r.x[l];
+}
+template <int L> static int mp_op_host(int op, const double* a, const double* b, double* out, long n) {
+    for (long k = 0; k < n; ++k) {
+        Real<L> x, y;
+        for (int l = 0; l < L; ++l) { x.x[l] = a[k * L + l]; y.x[l] = b[k * L + l]; }
+        Real<L> r = mp_apply<L>(op, x, y);
+        for (int l = 0; l < L; ++l) out[k * L + l] = r.x[l];
+    }
+    return TEUK_OK;
+}
+template <int L> static int mp_op_dev(int op, const double* a, const double* b, double* out, long n) {
+    double *da = nullptr, *db = nullptr, *dout = nullptr;
+    size_t bytes = (size_t)n * L * sizeof(double);
+    if (cudaMalloc(&da, bytes) != cudaSuccess || cudaMalloc(&db, bytes) != cudaSuccess ||
+        cudaMalloc(&dout, bytes) != cudaSuccess) {
+        cudaFree(da); cudaFree(db); cudaFree(dout);
+        return TEUK_ENOMEM;
+    }
+    cudaMemcpy(da, a, bytes, cudaMemcpyHostToDevice);
+    cudaMemcpy(db, b, bytes, cudaMemcpyHostToDevice);
+    mp_op_kernel<L><<<(unsigned)((n + 127) / 128), 128>>>(op, da, db, dout, n);
+    cudaError_t e = cudaMemcpy(out, dout, bytes, cudaMemcpyDeviceToHost);
+    cudaFree(da); cudaFree(db); cudaFree(dout);
+    return e == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+}
+extern "C" int teuk_test_mp_op(int op, int L, const double* a, const double* b, double* out, long n, int on_device) {
+    if (!a || !b || !out || n < 0 || op < 0 || op > 5 || (L != 2 && L != 4)) return TEUK_EINVAL;
+    if (L == 2) return on_device ? mp_op_dev<2>(op, a, b, out, n) : mp_op_host<2>(op, a, b, out, n);
+    return on_device ? mp_op_dev<4>(op, a, b, out, n) : mp_op_host<4>(op, a, b, out, n);
+}
+
+extern "C" int teuk_test_mp_fn(int fn, const double* a, double* out) {
+    if (!a || !out || fn < 0 || fn > 5) return TEUK_EINVAL;
+    static QConst qc = q_constants();
+    R4 x, r, t;
+    for (int l = 0; l < 4; ++l) x.x[l] = a[l];
+    switch (fn) {
+        case 0: r = q_exp(x, qc.ln2); break;
+        case 1: r = q_log(x, qc.ln2); break;
+        case 2: q_sincos(x, r, t); break;
+        case 3: q_sincos(x, t, r); break;
+        case 4: r = qc.pi; break;
+        default: r = qc.ln2; break;
+    }
+    for (int l = 0; l < 4; ++l) out[l] = r.x[l];
+    return TEUK_OK;
+}
+
+// FP64 issue-rate microbenchmark: 8 independent register chains per thread
+template <int KIND> __global__ void fp64_chain_kernel(long iters, double seed, double* sink) {
+    double x0 = seed, x1 = seed + 1, x2 = seed + 2, x3 = seed + 3, x4 = seed + 4, x5 = seed + 5, x6 = seed + 6, x7 = seed + 7;
+    const double m = 1.0000000001, c = 1e-9;
+    for (long i = 0; i < iters; ++i) {
+        if (KIND == 0) {
+            x0 = __fma_rn(x0, m, c); x1 = __fma_rn(x1, m, c); x2 = __fma_rn(x2, m, c); x3 = __fma_rn(x3, m, c);
+            x4 = __fma_rn(x4, m, c); x5 = __fma_rn(x5, m, c); x6 = __fma_rn(x6, m, c); x7 = __fma_rn(x7, m, c);
+        } else if (KIND == 1) {
+            x0 = __dadd_rn(x0, c); x1 = __dadd_rn(x1, c); x2 = __dadd_rn(x2, c); x3 = __dadd_rn(x3, c);
+            x4 = __dadd_rn(x4, c); x5 = __dadd_rn(x5, c); x6 = __dadd_rn(x6, c); x7 = __dadd_rn(x7, c);
+        } else {
+            x0 = __dmul_rn(x0, m); x1 = __dmul_rn(x1, m); x2 = __dmul_rn(x2, m); x3 = __dmul_rn(x3, m);
+            x4 = __dmul_rn(x4, m); x5 = __dmul_rn(x5, m); x6 = __dmul_rn(x6, m); x7 = __dmul_rn(x7, m);
+        }
+    }
+    double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 123.456) *sink = s;
+}
+extern "C" int teuk_bench_fp64(int kind, long iters, double* inst_per_s, void* cuda_stream) {
+    if (!inst_per_s || iters <= 0 || kind < 0 || kind > 2) return TEUK_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* sink = nullptr;
+    CK(cudaMalloc(&sink, 8));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    int blocks = sms * 8, threads = 256;
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, st);
+        if (kind == 0) fp64_chain_kernel<0><<<blocks, threads, 0, st>>>(iters, 1.0, sink);
+        else if (kind == 1) fp64_chain_kernel<1><<<blocks, threads, 0, st>>>(iters, 1.0, sink);
+        else fp64_chain_kernel<2><<<blocks, threads, 0, st>>>(iters, 1.0, sink);
+        cudaEventRecord(e1, st);
+        cudaEventSynchronize(e1);
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
+    *inst_per_s = (double)blocks * threads * 8.0 * (double)iters / (best * 1e-3);
+    return TEUK_OK;
+}

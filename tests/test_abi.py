@@ -1,0 +1,45 @@
+"""The C-ABI library loads and exports every symbol include/teuk.h declares (no compute calls)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "teuk.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(teuk_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_declares_the_north_star_calls():
+    syms = declared_symbols()
+    for name in ("teuk_create", "teuk_set_initial", "teuk_step", "teuk_read", "teuk_observe"):
+        assert name in syms
+
+
+def test_library_exports_every_declared_symbol():
+    so = os.path.join(ROOT, "paper_1006_0663_b200", "libteuk.so")
+    if not os.path.exists(so):
+        pytest.skip("libteuk.so not built (run __graft_entry__.build())")
+    lib = ctypes.CDLL(so)
+    for name in declared_symbols():
+        assert hasattr(lib, name), name
+    from paper_1006_0663_b200 import teuk
+    assert sorted(teuk.SIGNATURES) == declared_symbols()
+
+
+def test_argument_validation_without_gpu():
+    teuk = pytest.importorskip("paper_1006_0663_b200.teuk")
+    out = ctypes.c_size_t(0)
+    assert teuk.lib.teuk_workspace_bytes(2, 16, 1, 0, ctypes.byref(out)) == teuk.EINVAL
+    assert teuk.lib.teuk_workspace_bytes(512, 16, 3, 0, ctypes.byref(out)) == teuk.EINVAL
+    assert teuk.lib.teuk_workspace_bytes(512, 16, 1, 2000, ctypes.byref(out)) == teuk.OK
+    # two state buffers + 16 coefficient planes of 16 x 512 doubles at least
+    assert out.value >= (8 + 16) * 512 * 16 * 8
+    assert teuk.workspace_bytes(16384, 64, 2, 0) >= 2 * (8 + 16) * 16384 * 64 * 8
+    h = ctypes.c_void_p()
+    assert teuk.lib.teuk_create(1.0, 1.0, 0, 0, 64, 8, -10.0, 10.0, 0.1, 1, None, 0, 0, None, ctypes.byref(h)) == teuk.EINVAL
+    assert teuk.lib.teuk_strerror(teuk.ESTATE).decode().startswith("call not valid")
