@@ -1,0 +1,308 @@
+#!/usr/bin/env python
+"""bench.py — Teukolsky grid-point updates/s on B200 (BASELINE.json metric).
+
+A "step" is one full Lax-Wendroff iteration (half step + full step + boundary/polar conditions + observer
+sample) over the whole grid.  Default workload at N = 1: BASELINE.json configs[1]
+(Kerr a=0.9, s=-2, m=2, fp64, 16384 x 64), with dd (configs[2]) and qd (configs[3]) reported beside it in
+`per_precision`.  One JSON line on stdout (rank 0).  See DESIGN.md §7 for every field.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--precision 1|2|4] [--workload cfg2|cfg3|cfg4|sweep:NRxNT]
+  python bench.py --impl reference ...     # the oracle on the host cores (same metric, bounded sample)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+ALG_BYTES_PER_UPDATE = {1: 192.0, 2: 384.0, 4: 768.0}     # 4L read + 4L write + 16L coefficients, x 8 B
+FALLBACK_HBM_GBS = 6650.0
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=200)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--no-extra", action="store_true", help="skip the dd/qd side measurements and the cpu baseline")
+    ap.add_argument("--option", action="append", default=[], help="key=value passed to teuk_set_option")
+    return ap.parse_args()
+
+
+def workload(name: str):
+    from paper_1006_0663_b200 import inputs
+    if name.startswith("cfg"):
+        return inputs.config(int(name[3:]))
+    if name.startswith("sweep:"):
+        dims, _, prec = name[6:].partition(":")
+        nr, nt = dims.lower().split("x")
+        return inputs.sweep_cell(int(nr), int(nt), int(prec or 1))
+    raise SystemExit(f"unknown workload {name}")
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._pump, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = max(mx, float(r[1]))
+                for n, v in zip(names, r[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores; each step a bounded sample (a radial
+    window of the workload's grid, same dr*, dtheta, dt, coefficients)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle
+    from paper_1006_0663_b200 import inputs
+    import numpy as np
+    w = workload(args.workload)
+    n_win = min(w.n_r, 2048)
+    i_lo = max(0, int((inputs.pulse_parameters(w)[0] - w.rstar_min) / w.dr) - n_win // 2)
+    cores = oracle.set_threads(0)
+    o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win)
+    u0 = inputs.initial_state(w)[..., i_lo:i_lo + n_win]
+    o.set_initial(np.ascontiguousarray(u0))
+    per = {1: 1, 2: 1, 4: 1}[w.precision]
+    o.step(args.warmup * per if w.precision == 1 else min(args.warmup, 2))
+    steps = args.steps if w.precision == 1 else max(1, min(args.steps, 20))
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    val = n_win * w.n_theta * steps / dt
+    sample = f"radial window of {n_win} of {w.n_r} columns x {w.n_theta} rows, {steps} steps"
+    line = {"impl": "reference", "metric": "Teukolsky grid-point updates/s", "value": val, "unit": "updates/s",
+            "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": {1: "f64", 2: "f64x2 (double-double)", 4: "f64x4 (quad-double)"}[w.precision],
+            "data": "synthetic", "config": {"workload": w.name, "n_r": w.n_r, "n_theta": w.n_theta, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": "updates/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def make_solver(teuk, w, options, obs_capacity):
+    g = teuk.Teuk.from_workload(w, obs_capacity=obs_capacity)
+    for kv in options:
+        k, _, v = kv.partition("=")
+        g.set_option(k, float(v))
+    ro, to = w.observer
+    g.set_observer(ro, to, obs_capacity)
+    return g
+
+
+def time_device(torch, teuk, w, steps, warmup, options, dist=None):
+    """inputs resident in HBM; CUDA events on the stream the kernels are launched on."""
+    from paper_1006_0663_b200 import inputs
+    g = make_solver(teuk, w, options, warmup + steps)
+    u0 = torch.from_numpy(inputs.initial_state(w)).to(g.device)
+    g.set_initial(u0)
+    g.step(warmup)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    n0 = g.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(g.stream)
+    g.step(steps)
+    e1.record(g.stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        dist.barrier()
+    launches = g.launch_count() - n0
+    geom = g.step_geometry()
+    ser = g.observe(4, allow_nonfinite=True)
+    finite = bool(torch.isfinite(g.read_device()).all().item()) and g.last_observe_status == 0
+    g.close()
+    return ms, launches, geom, finite
+
+
+def time_e2e(torch, teuk, w, steps, options):
+    """same job through the C ABI with HOST buffers: teuk_set_initial (H2D from pinned memory) + teuk_step +
+    teuk_read (D2H into pinned memory) all inside the timed region."""
+    from paper_1006_0663_b200 import inputs
+    g = make_solver(teuk, w, options, steps)
+    host_in = torch.from_numpy(inputs.initial_state(w)).pin_memory()
+    host_out = torch.empty((4, w.precision, w.n_theta, w.n_r), dtype=torch.float64).pin_memory()
+    g.set_initial_pinned(host_in)
+    g.step(min(steps, 64))
+    g.read_pinned(host_out)                     # warm-up of the whole call sequence
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    g.set_initial_pinned(host_in)
+    g.step(steps)
+    g.read_pinned(host_out)                     # synchronises the stream
+    dt = time.perf_counter() - t0
+    g.close()
+    return dt, host_in.numel() * 8, host_out.numel() * 8
+
+
+def cpu_baseline(w):
+    """the oracle as it stands, on this box's host cores, on a bounded sample of the same workload."""
+    import numpy as np
+    from oracle import oracle
+    from paper_1006_0663_b200 import inputs
+    n_win = min(w.n_r, 1024)
+    i_lo = max(0, int((inputs.pulse_parameters(w)[0] - w.rstar_min) / w.dr) - n_win // 2)
+    cores = oracle.set_threads(0)
+    o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win)
+    o.set_initial(np.ascontiguousarray(inputs.initial_state(w)[..., i_lo:i_lo + n_win]))
+    steps = {1: 400, 2: 8, 4: 4}[w.precision]
+    o.step(2)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return {"value": n_win * w.n_theta * steps / dt, "unit": "updates/s", "cores": cores, "kind": "oracle",
+            "sample": f"radial window of {n_win} of {w.n_r} columns x {w.n_theta} rows, {steps} steps, {w.name}"}
+
+
+def load_traffic(name):
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p)).get(name)
+    except Exception:
+        return None
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    d = None
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        d = dist
+    from paper_1006_0663_b200 import teuk
+    w = workload(args.workload)
+    L = w.precision
+    points = w.n_r * w.n_theta
+    with ClockSampler(local) as cs:
+        ms, launches, geom, finite = time_device(torch, teuk, w, args.steps, args.warmup, args.option, d)
+    clocks = cs.summary()
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if d is not None:
+        d.all_reduce(t, op=dist.ReduceOp.MAX)                     # max over ranks; replicas only, no data-path collective
+    ms_max = float(t.item())
+    value = world * points * args.steps / (ms_max * 1e-3)
+    e2e_dt, h2d, d2h = time_e2e(torch, teuk, w, args.steps, args.option)
+    te = torch.tensor([e2e_dt], dtype=torch.float64, device="cuda")
+    if d is not None:
+        d.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_val = world * points * args.steps / float(te.item())
+    if rank != 0:
+        if d is not None:
+            d.destroy_process_group()
+        return
+    peak, peak_src = measured_peaks()
+    alg_bytes = ALG_BYTES_PER_UPDATE[L] * points
+    achieved = alg_bytes / (ms / args.steps * 1e-3) / 1e9
+    line = {
+        "metric": "Teukolsky grid-point updates/s", "value": value, "unit": "updates/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": {1: "f64", 2: "f64x2 (double-double)", 4: "f64x4 (quad-double)"}[L], "data": "synthetic",
+        "config": {"workload": w.name, "M": w.M, "a": w.a, "s": w.s, "m": w.m, "n_r": w.n_r, "n_theta": w.n_theta,
+                   "dt_over_dr": w.dt / w.dr, "precision_limbs": L, "parallelism": f"replicas x{world}",
+                   "l2": "working set (2 state copies + 16L coefficient planes = %d MiB) exceeds the 126 MB L2; no flush"
+                         % (24 * L * points * 8 // 2 ** 20),
+                   "geometry": geom, "finite": finite},
+        "clocks": clocks,
+        "e2e": {"value": e2e_val, "unit": "updates/s", "h2d_bytes_per_step": h2d / args.steps,
+                "d2h_bytes_per_step": d2h / args.steps,
+                "note": "teuk_set_initial(host) + teuk_step(K) + teuk_read(host) timed by wall clock; bytes are the whole "
+                        "state once per K-step call divided by K"},
+        "gpu_launches": launches,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": load_traffic(f"{w.name}"), "peak_source": peak_src, "kernel": f"step_kernel<{L}>",
+                     "algorithmic_bytes_per_update": ALG_BYTES_PER_UPDATE[L]},
+    }
+    if not args.no_extra and world == 1:
+        per = {}
+        fp = {k: teuk.bench_fp64(k) for k in ("dfma", "dadd", "dmul")}
+        for name, k_steps in (("cfg3", max(50, args.steps // 10)), ("cfg4", max(50, args.steps // 10))):
+            wx = workload(name)
+            msx, lx, gx, fx = time_device(torch, teuk, wx, k_steps, 20, args.option)
+            per[name] = {"precision_limbs": wx.precision, "n_r": wx.n_r, "n_theta": wx.n_theta, "steps": k_steps,
+                         "updates_per_s": wx.n_r * wx.n_theta * k_steps / (msx * 1e-3), "ms_per_step": msx / k_steps,
+                         "geometry": gx, "finite": fx}
+        line["per_precision"] = per
+        line["fp64_pipe_peak_inst_per_s"] = fp
+        line["cpu_baseline"] = cpu_baseline(w)
+    print(json.dumps(line), flush=True)
+    if d is not None:
+        d.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,260 @@
+"""GPU parity tests (pin P10): the CUDA path through the C ABI (paper_1006_0663_b200.teuk) against the
+oracle (oracle/) element by element on the same seeded inputs.  Tolerances are BASELINE.json's relative
+L-infinity bounds (reading A17): 1e-12 fp64, 1e-27 dd, 1e-55 qd."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import mp_ref, oracle
+from paper_1006_0663_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+TOL = {1: 1e-12, 2: 1e-27, 4: 1e-55}
+
+
+@pytest.fixture(scope="module")
+def teuk():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1006_0663_b200 import teuk as t
+    return t
+
+
+def run_gpu(teuk, w, u0, steps, precision=None, observer=None, options=None):
+    L = precision or w.precision
+    g = teuk.Teuk.from_workload(w, precision=L, obs_capacity=steps if observer else 0)
+    for k, v in (options or {}).items():
+        g.set_option(k, v)
+    if observer:
+        g.set_observer(observer[0], observer[1], steps)
+    g.set_initial(u0)
+    g.step(steps)
+    return g
+
+
+def run_oracle(w, u0, steps, precision=None, observer=None, i_lo=0, n_win=None):
+    o = oracle.Oracle.from_workload(w, precision=precision or w.precision, i_lo=i_lo, n_win=n_win)
+    if observer:
+        o.set_observer(observer[0], observer[1], steps)
+    o.set_initial(u0)
+    o.step(steps)
+    return o
+
+
+def series_err(a, b):
+    """observer series [n][4][L]: max over samples of |F_gpu - F_ref| / max |F_ref| per complex field"""
+    a4 = np.ascontiguousarray(np.transpose(a, (1, 2, 0)))
+    b4 = np.ascontiguousarray(np.transpose(b, (1, 2, 0)))
+    return oracle.rel_linf(a4, b4)
+
+
+# ------------------------------------------------------------------------------- arithmetic layer on device
+@pytest.mark.parametrize("L", [2, 4])
+@pytest.mark.parametrize("op", ["add", "sub", "mul", "div", "sqrt", "mul_d"])
+def test_device_arithmetic_bitwise_equals_host_build(teuk, L, op):
+    rng = np.random.default_rng(7 + L)
+    n = 4096
+    a = rng.uniform(0.5, 2.0, size=(n, L)) * (2.0 ** (-54.0 * np.arange(L)))[None, :] * rng.choice([-1, 1], size=(n, L))
+    b = rng.uniform(0.5, 2.0, size=(n, L)) * (2.0 ** (-54.0 * np.arange(L)))[None, :] * rng.choice([-1, 1], size=(n, L))
+    if op == "sqrt":
+        a[:, 0] = np.abs(a[:, 0])
+    b[::3] = -a[::3] * (1 + 2.0 ** -70)                       # cancellation rows
+    host = teuk.test_mp_op(op, L, a, b, on_device=False)
+    dev = teuk.test_mp_op(op, L, a, b, on_device=True)
+    assert np.array_equal(host, dev)
+
+
+# ------------------------------------------------------------------------------- setup: r(r*) and tables
+@pytest.mark.parametrize("cfg", [1, 2, 4])
+def test_radial_inversion_matches_mpmath(teuk, cfg):
+    import mpmath as mp
+    w = inputs.config(cfg).scaled(n_r=257)
+    g = teuk.Teuk.from_workload(w)
+    r, d = g.radial()
+    with mp.workdps(110):
+        lo = mp.mpf(w.rstar_min)
+        dr = (mp.mpf(w.rstar_max) - lo) / (w.n_r - 1)
+        for k in (0, 1, 2, 17, 128, 255, 400, 512):
+            rr, dd = mp_ref.r_of_rstar(lo + k * dr / 2, w.M, w.a)
+            assert abs(mp_ref.from_limbs(r[k]) - rr) / rr < mp.mpf(10) ** -58
+            assert abs(mp_ref.from_limbs(d[k]) - dd) / dd < mp.mpf(10) ** -58, (k, mp.nstr(dd, 5))
+
+
+@pytest.mark.parametrize("cfg,L", [(1, 1), (2, 1), (2, 2), (4, 4)])
+def test_coefficient_tables_match_oracle(teuk, cfg, L):
+    w = inputs.config(cfg).scaled(n_r=129)
+    g = teuk.Teuk.from_workload(w, precision=L)
+    o = oracle.Oracle.from_workload(w, precision=L)
+    eps = {1: 2.0 ** -52, 2: 2.0 ** -102, 4: 2.0 ** -198}[L]
+    for half in (False, True):
+        tg, to = g.tables(half), o.tables(half)
+        for q in range(8):
+            diff, _ = oracle._limb_diff(tg[q], to[q])
+            scale = np.maximum(np.abs(to[q, 0]).ravel(), np.abs(to[:, 0]).max(axis=0).ravel() / 64)
+            assert np.all(np.abs(diff) <= 8 * eps * scale), (half, q, float(np.max(np.abs(diff) / scale)))
+
+
+# ------------------------------------------------------------------------------- full runs on small / ragged grids
+def test_config1_full_run_fp64(teuk):
+    w = inputs.config(1)
+    u0 = inputs.initial_state(w)
+    g = run_gpu(teuk, w, u0, w.steps, observer=w.observer)
+    o = run_oracle(w, u0, w.steps, observer=w.observer)
+    err = oracle.rel_linf(g.read(), o.read())
+    print("cfg1 final-state error", err)
+    assert max(err.values()) <= TOL[1]
+    serr = series_err(g.observe(w.steps), o.observe(w.steps))
+    print("cfg1 observer error", serr)
+    assert max(serr.values()) <= TOL[1]
+    assert g.steps_done() == w.steps
+
+
+@pytest.mark.parametrize("L,n_r,n_t,steps,base", [(1, 203, 13, 300, 2), (2, 203, 13, 200, 2), (4, 131, 11, 80, 2),
+                                                  (2, 300, 40, 60, 4), (4, 150, 32, 40, 4), (1, 1000, 70, 100, 2)])
+def test_ragged_grids_all_precisions(teuk, L, n_r, n_t, steps, base):
+    """sizes that span several tiles with ragged tails in both directions; generic complex state with
+    every field and limb populated; Kerr coefficients (cfg 2 physics) or cfg 4 physics"""
+    w0 = inputs.config(base)
+    lo, hi = -30.0, 60.0
+    w = w0.scaled(n_r=n_r, n_theta=n_t, rstar_min=lo, rstar_max=hi, precision=L)
+    w = w.scaled(dt_override=inputs.stable_dt(w))
+    u0 = inputs.random_state(n_r, n_t, L, seed=100 + L)
+    obs = (10.3, 1.1)
+    g = run_gpu(teuk, w, u0, steps, observer=obs)
+    o = run_oracle(w, u0, steps, observer=obs)
+    err = oracle.rel_linf(g.read(), o.read())
+    serr = series_err(g.observe(steps), o.observe(steps))
+    print(L, n_r, n_t, "state", err, "observer", serr)
+    assert max(err.values()) <= TOL[L]
+    assert max(serr.values()) <= TOL[L]
+
+
+@pytest.mark.parametrize("ti,tj", [(8, 4), (32, 16), (64, 8), (16, 64)])
+def test_tile_shapes_give_identical_results(teuk, ti, tj):
+    w = inputs.config(2).scaled(n_r=150, n_theta=24, rstar_min=-30.0, rstar_max=60.0, precision=2)
+    w = w.scaled(dt_override=inputs.stable_dt(w))
+    u0 = inputs.random_state(w.n_r, w.n_theta, 2, seed=9)
+    ref = run_gpu(teuk, w, u0, 30).read()
+    got = run_gpu(teuk, w, u0, 30, options={"tile_i": ti, "tile_j": tj}).read()
+    assert np.array_equal(ref, got)
+
+
+# ------------------------------------------------------------------------------- full-size configs (bench launch geometry)
+@pytest.mark.parametrize("cfg,steps_gpu,k", [(2, 300, 12), (3, 120, 8), (4, 100, 6)])
+def test_full_size_configs_windowed(teuk, cfg, steps_gpu, k):
+    """BASELINE.json configs 2-4 at full grid size in the launch configuration bench.py times: the GPU
+    runs steps_gpu iterations, then k more; the oracle advances sampled radial windows of the GPU's
+    state by the same k iterations (domain of dependence: interior of the window is exact)."""
+    w = inputs.config(cfg)
+    L = w.precision
+    u0 = inputs.initial_state(w)
+    g = run_gpu(teuk, w, u0, steps_gpu)
+    mid = g.read()
+    assert np.isfinite(mid).all() and np.abs(mid[0, 0]).max() > 1e-3
+    g.step(k)
+    fin = g.read()
+    c = inputs.pulse_parameters(w)[0]
+    i_c = int((c - w.rstar_min) / w.dr)
+    n_win = 96
+    worst = {}
+    for i_lo in (0, i_c - n_win // 2, i_c + 3 * n_win, w.n_r - n_win):
+        o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win)
+        o.set_initial(np.ascontiguousarray(mid[..., i_lo:i_lo + n_win]))
+        o.step(k)
+        ref = o.read()
+        a, b = k + 1, n_win - k - 1
+        if i_lo == 0:
+            a = 0                                   # true Dirichlet wall: the window edge IS the boundary
+        if i_lo + n_win == w.n_r:
+            b = n_win
+        sl = slice(a, b)
+        scale_ref = np.zeros_like(fin)              # normalise by the global field maximum (A17)
+        got = np.ascontiguousarray(fin[..., i_lo:i_lo + n_win][..., sl])
+        want = np.ascontiguousarray(ref[..., sl])
+        diffs = {}
+        for name, (re, im) in {"Phi": (0, 1), "Pi": (2, 3)}.items():
+            dre, _ = oracle._limb_diff(got[re], want[re])
+            dim, _ = oracle._limb_diff(got[im], want[im])
+            den = np.hypot(fin[re, 0], fin[im, 0]).max()
+            diffs[name] = float(np.hypot(dre, dim).max() / den)
+        worst[i_lo] = diffs
+        assert max(diffs.values()) <= TOL[L], (i_lo, diffs)
+    print(cfg, worst)
+
+
+def test_config2_prefix_full_grid_fp64(teuk):
+    """config 2 at full size against the full-grid oracle for a 150-step prefix (observer included)."""
+    w = inputs.config(2)
+    u0 = inputs.initial_state(w)
+    steps = 150
+    g = run_gpu(teuk, w, u0, steps, observer=w.observer)
+    o = run_oracle(w, u0, steps, observer=w.observer)
+    err = oracle.rel_linf(g.read(), o.read())
+    print("cfg2 prefix", err)
+    assert max(err.values()) <= TOL[1]
+    serr = series_err(g.observe(steps), o.observe(steps))
+    assert max(serr.values()) <= TOL[1] or np.abs(o.observe(steps)).max() < 1e-300
+
+
+# ------------------------------------------------------------------------------- invariants and edge cases
+@pytest.mark.parametrize("L", [1, 2, 4])
+def test_gpu_exact_invariants(teuk, L):
+    w = inputs.config(1).scaled(n_r=96, precision=L)
+    u0 = inputs.initial_state(w)
+    g = run_gpu(teuk, w, u0, 50)
+    u = g.read()
+    assert np.array_equal(u, u[:, :, ::-1, :])                      # reflection symmetry (A12), bitwise
+    assert not u[..., 0].any() and not u[..., -1].any()             # Dirichlet rows
+    assert not u[1].any() and not u[3].any()                        # real data stay real for a = 0
+    # power-of-two linearity, bitwise
+    g2 = run_gpu(teuk, w, u0 * 2.0 ** 7, 50)
+    assert np.array_equal(g2.read(), u * 2.0 ** 7)
+    # checkpoint / restart and graph / no-graph equivalence, bitwise
+    g3 = run_gpu(teuk, w, u0, 21, options={"graph_steps": 0})
+    mid = g3.read()
+    g4 = run_gpu(teuk, w, mid, 29, options={"graph_steps": 4})
+    assert np.array_equal(g4.read(), u)
+
+
+def test_edge_cases_and_errors(teuk):
+    import ctypes
+    # smallest legal grid, odd m, zero steps
+    w = inputs.config(1).scaled(n_r=3, n_theta=2, m=1)
+    u0 = inputs.random_state(3, 2, 1, seed=1)
+    g = run_gpu(teuk, w, u0, 0)
+    assert g.steps_done() == 0
+    g.step(5)
+    o = run_oracle(w, u0, 5)
+    assert max(oracle.rel_linf(g.read(), o.read()).values()) <= TOL[1] or not o.read().any()
+    # odd m on a real grid
+    w = inputs.config(2).scaled(n_r=90, n_theta=10, m=1, s=-1, rstar_min=-20.0, rstar_max=40.0)
+    w = w.scaled(dt_override=inputs.stable_dt(w))
+    u0 = inputs.random_state(90, 10, 1, seed=2)
+    g = run_gpu(teuk, w, u0, 40)
+    o = run_oracle(w, u0, 40)
+    assert max(oracle.rel_linf(g.read(), o.read()).values()) <= TOL[1]
+    # state errors
+    h = teuk.Teuk.from_workload(w)
+    with pytest.raises(teuk.TeukError) as e:
+        h.step(1)
+    assert e.value.code == teuk.ESTATE
+    with pytest.raises(teuk.TeukError) as e:
+        h.set_observer(1e9, 1.0, 0)
+    assert e.value.code == teuk.EINVAL
+    h.set_initial(u0)
+    with pytest.raises(teuk.TeukError) as e:
+        h.set_option("graph_steps", 8)
+    assert e.value.code == teuk.ESTATE
+    with pytest.raises(teuk.TeukError):
+        teuk.Teuk(1.0, 1.5, 0, 0, 64, 8, -10.0, 10.0, 0.1, 1)
+    # non-finite detection is sticky and reported
+    bad = u0.copy()
+    bad[0, 0, 5, 40] = np.inf
+    hb = teuk.Teuk.from_workload(w, obs_capacity=8)
+    hb.set_observer(w.rstar_min + 40.2 * w.dr, (5.5) * math.pi / w.n_theta, 8)
+    hb.set_initial(bad)
+    hb.step(3)
+    hb.observe(8, allow_nonfinite=True)
+    assert hb.last_observe_status == teuk.ENONFINITE
