@@ -12,7 +12,7 @@
  *    untouched on error.  One handle = one CUDA stream; handles are not thread-safe.
  *  - Pointers named host_* are HOST memory owned by the caller; d_workspace is DEVICE memory owned
  *    by the caller (e.g. a torch tensor) that must outlive the handle; cuda_stream is a borrowed
- *    cudaStream_t (NULL = the legacy default stream).
+ *    cudaStream_t (NULL = the legacy default stream, on which CUDA graphs are not used).
  */
 #ifndef TEUK_H
 #define TEUK_H

@@ -388,7 +388,8 @@ extern "C" int teuk_step(teuk_ctx* c, long n) {
     if (!c || n < 0) return TEUK_EINVAL;
     if (!c->have_init) return TEUK_ESTATE;
     long left = n;
-    const int K = c->graph_steps;
+    // the legacy default stream cannot be captured: plain launches there
+    const int K = (c->stream == nullptr || c->stream == cudaStreamLegacy) ? 0 : c->graph_steps;
     while (K > 0 && left >= K) {
         if (!c->graph[c->cur]) {
             int rc = build_graph(c, c->cur);

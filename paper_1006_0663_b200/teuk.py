@@ -89,7 +89,8 @@ class Teuk:
         self.device = torch.device(device)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            # own non-default stream unless one is given (the legacy default stream cannot be graph-captured)
+            self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
             base = self.workspace.data_ptr()
             self._ws_ptr = (base + 255) // 256 * 256
             self.h = _h()
@@ -125,6 +126,7 @@ class Teuk:
         else:
             t = planes.contiguous()
             assert t.is_cuda and t.dtype == self.torch.float64
+            self.stream.wait_stream(self.torch.cuda.current_stream(self.device))   # t was produced there
             limbs_in = 1 if t.dim() == 3 else t.shape[1]
             assert t.shape[0] == 4 and tuple(t.shape[-2:]) == (self.n_theta, self.n_r)
             _chk(lib.teuk_set_initial_device(self.h, C.c_void_p(t.data_ptr()), limbs_in), "teuk_set_initial_device")
@@ -151,6 +153,7 @@ class Teuk:
         if t is None:
             t = self.torch.empty((4, self.L, self.n_theta, self.n_r), dtype=self.torch.float64, device=self.device)
         _chk(lib.teuk_read_device(self.h, C.c_void_p(t.data_ptr())), "teuk_read_device")
+        self.torch.cuda.current_stream(self.device).wait_stream(self.stream)   # consumers run there
         return t
 
     def observe(self, max_samples: int, allow_nonfinite=False):
