@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libteuk.so")
 SOURCES = ["teuk.cu"]
-HEADERS = ["mp.cuh", "setup_math.cuh", "setup_kernels.cuh", "step_kernel.cuh"]
+HEADERS = ["mp.cuh", "setup_math.cuh", "setup_kernels.cuh", "step_kernel.cuh", "step_kernel_tma.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=true",
               "-Xcompiler", "-fPIC,-O2,-ffp-contract=off", "-shared"]
 

@@ -64,9 +64,15 @@ template <int L> __device__ __forceinline__ Real<L> sgn(const Real<L>& a, double
 // One sub-step at one point.  T: tile accessor giving Real<L> at (component, row offset, column).
 // lo/hi are the two radial neighbour columns in the tile; rows jm/jp are the theta neighbours
 // (already mirrored) with signs sm/sp.
-template <int L, class Tile>
+template <int L> struct GlobalCoef {       // coefficient q straight from the global planes (coalesced, read-only path)
+    const double* __restrict__ p;
+    long stride, idx;
+    __device__ __forceinline__ Real<L> get(int q) const { return Ld<L>::g(p + (long)q * L * stride, stride, idx); }
+};
+
+template <int L, class Tile, class Coef>
 __device__ __forceinline__ void substep(const Tile& t, int row, int rm, int rp, double sm, double sp, int clo, int chi,
-                                        const double* __restrict__ coef, long cstride, long cidx, const Real<L>& cjv,
+                                        const Coef& cf, const Real<L>& cjv,
                                         double tq, bool half, const Real<L> base_in[4], Real<L> out[4]) {
     Real<L> sg[4], dl[4];
 #pragma unroll
@@ -85,14 +91,14 @@ __device__ __forceinline__ void substep(const Tile& t, int row, int rm, int rp, 
         Real<L> first = mul(cjv, sub(up, dn));
         lam[c] = add(second, first);
     }
-    Real<L> c0 = Ld<L>::g(coef + 0 * L * cstride, cstride, cidx);
-    Real<L> c1 = Ld<L>::g(coef + 1 * L * cstride, cstride, cidx);
-    Real<L> c2 = Ld<L>::g(coef + 2 * L * cstride, cstride, cidx);
-    Real<L> c3 = Ld<L>::g(coef + 3 * L * cstride, cstride, cidx);
-    Real<L> c4 = Ld<L>::g(coef + 4 * L * cstride, cstride, cidx);
-    Real<L> c5 = Ld<L>::g(coef + 5 * L * cstride, cstride, cidx);
-    Real<L> c6 = Ld<L>::g(coef + 6 * L * cstride, cstride, cidx);
-    Real<L> c7 = Ld<L>::g(coef + 7 * L * cstride, cstride, cidx);
+    Real<L> c0 = cf.get(0);
+    Real<L> c1 = cf.get(1);
+    Real<L> c2 = cf.get(2);
+    Real<L> c3 = cf.get(3);
+    Real<L> c4 = cf.get(4);
+    Real<L> c5 = cf.get(5);
+    Real<L> c6 = cf.get(6);
+    Real<L> c7 = cf.get(7);
     // tau * S_Pi, summed in the printed order of S: -alpha Pi + gamma Phi_* + kappa Lam - W Phi
     Real<L> sR = neg(sub(mul(c1, sg[2]), mul(c2, sg[3])));
     Real<L> sI = neg(add(mul(c1, sg[3]), mul(c2, sg[2])));
@@ -157,8 +163,8 @@ __global__ void __launch_bounds__(256) step_kernel(StepParams P) {
         if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
         Real<L> cjv = Ld<L>::g(P.cj, nt, jh);
         Real<L> out[4];
-        substep<L>(ut, jh, rm, rp, sm, sp, tc, tc + 1, P.coef_h, P.plane, (long)jh * P.pitch + ih, cjv, P.tq_half,
-                   true, out, out);
+        GlobalCoef<L> cf{P.coef_h, P.plane, (long)jh * P.pitch + ih};
+        substep<L>(ut, jh, rm, rp, sm, sp, tc, tc + 1, cf, cjv, P.tq_half, true, out, out);
 #pragma unroll
         for (int c = 0; c < 4; ++c)
 #pragma unroll
@@ -186,8 +192,8 @@ __global__ void __launch_bounds__(256) step_kernel(StepParams P) {
             for (int c = 0; c < 4; ++c) base[c] = ut.get(c, j, tc + 1);
             Real<L> cjv = Ld<L>::g(P.cj, nt, j);
             // h columns: tile col tc <-> i - 1/2, tc + 1 <-> i + 1/2
-            substep<L>(ht, j, rm, rp, sm, sp, tc, tc + 1, P.coef_i, P.plane, (long)j * P.pitch + i, cjv, P.tq_full,
-                       false, base, out);
+            GlobalCoef<L> cf{P.coef_i, P.plane, (long)j * P.pitch + i};
+            substep<L>(ht, j, rm, rp, sm, sp, tc, tc + 1, cf, cjv, P.tq_full, false, base, out);
         }
         long g = (long)j * P.pitch + i;
 #pragma unroll

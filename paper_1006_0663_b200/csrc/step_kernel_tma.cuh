@@ -1,0 +1,183 @@
+// fp64 step kernel for sm_100a with TMA staging (the HBM-bound precision).  Same arithmetic as
+// step_kernel<1> (it calls the same substep<1>), different data movement:
+//   * ONE elected thread issues three 3-D tiled TMA loads (cp.async.bulk.tensor) per block: the u^n tile
+//     with its halo (4 planes), the half-point coefficient tile (8 planes) and the integer-point
+//     coefficient tile (8 planes).  Out-of-range columns/rows are zero-filled by the TMA unit, which
+//     supplies the radial Dirichlet halo for free; polar ghosts stay mirrored reads.
+//   * all ~90 KB a block needs are in flight from its first instruction (two mbarriers: the full-step
+//     coefficients may land while the half step computes), so HBM latency is paid once per block and
+//     hidden by the co-resident block(s);
+//   * tile sizes are compile-time, so index arithmetic folds into constants (the generic kernel spends
+//     ~900 thread instructions per update, mostly integer).
+#pragma once
+#include <cuda.h>
+
+#include <cstdint>
+
+#include "step_kernel.cuh"
+
+namespace tk {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int x, int y, int z, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            smem_u32(dst)),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
+        : "memory");
+}
+
+template <int TI, int TJ> struct TmaGeom {
+    // TMA needs a 16-byte aligned start in the innermost dimension, i.e. an EVEN first column: both haloed boxes
+    // start at column i0 - 2 (one unused leading column) instead of i0 - 1.
+    static constexpr int UC = TI + 4, UR = TJ + 4, HC = TI + 1, HR = TJ + 2, CC = TI + 2;
+    static constexpr int a128(int v) { return (v + 127) / 128 * 128; }
+    static constexpr int US_B = a128(4 * UR * UC * 8);        // u tile   [4][UR][UC], columns i0-2 .. i0+TI+1
+    static constexpr int CH_B = a128(8 * HR * CC * 8);        // coef_h   [8][HR][CC], half points i0-2 .. i0+TI-1
+    static constexpr int CI_B = a128(8 * TJ * TI * 8);        // coef_i   [8][TJ][TI]
+    static constexpr int HS_B = a128(4 * HR * HC * 8);        // h tile   [4][HR][HC]
+    static constexpr int TOTAL = US_B + CH_B + CI_B + HS_B + 128;
+};
+
+template <int ROWS, int COLS> struct CTile {       // compile-time shaped smem tile of fp64 planes
+    const double* p;
+    int row0;
+    __device__ __forceinline__ R1 get(int c, int grow, int col) const {
+        R1 r;
+        r.x[0] = p[c * ROWS * COLS + (grow - row0) * COLS + col];
+        return r;
+    }
+};
+template <int ROWS, int COLS> struct CCoef {
+    const double* p;     // already offset to (row, col)
+    __device__ __forceinline__ R1 get(int q) const {
+        R1 r;
+        r.x[0] = p[q * ROWS * COLS];
+        return r;
+    }
+};
+
+template <int TI, int TJ>
+__global__ void __launch_bounds__(256) step_kernel_f64_tma(const __grid_constant__ CUtensorMap tm_u,
+                                                          const __grid_constant__ CUtensorMap tm_ch,
+                                                          const __grid_constant__ CUtensorMap tm_ci, StepParams P) {
+    using G = TmaGeom<TI, TJ>;
+    constexpr int UC = G::UC, UR = G::UR, HC = G::HC, HR = G::HR, CC = G::CC;
+    extern __shared__ __align__(128) unsigned char raw[];
+    __shared__ __align__(8) uint64_t bar[2];
+    unsigned char* base = (unsigned char*)(((uintptr_t)raw + 127) & ~(uintptr_t)127);
+    double* us = (double*)base;
+    double* chs = (double*)(base + G::US_B);
+    double* cis = (double*)(base + G::US_B + G::CH_B);
+    double* hs = (double*)(base + G::US_B + G::CH_B + G::CI_B);
+    const int i0 = blockIdx.x * TI, j0 = blockIdx.y * TJ;
+    const int nt = P.n_theta, nr = P.n_r;
+    const int tid = threadIdx.x;
+
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&bar[0], 4 * UR * UC * 8 + 8 * HR * CC * 8);
+        tma_load_3d(us, &tm_u, i0 - 2, j0 - 2, 0, &bar[0]);
+        tma_load_3d(chs, &tm_ch, i0 - 2, j0 - 1, 0, &bar[0]);
+        mbar_expect_tx(&bar[1], 8 * TJ * TI * 8);
+        tma_load_3d(cis, &tm_ci, i0, j0, 0, &bar[1]);
+    }
+    mbar_wait(&bar[0], 0);
+
+    CTile<UR, UC> ut{us, j0 - 2};
+    // ---- half step, Eq. (13)
+#pragma unroll
+    for (int k = 0; k < (HR * HC + 255) / 256; ++k) {
+        int idx = tid + k * 256;
+        if (idx < HR * HC) {
+            int tr = idx / HC, tc = idx - tr * HC;
+            int ih = i0 - 1 + tc, jh = j0 - 1 + tr;
+            if (ih >= 0 && ih <= nr - 2 && jh >= 0 && jh < nt) {
+                int rm = jh - 1, rp = jh + 1;
+                double sm = 1.0, sp = 1.0;
+                if (rm < 0) { rm = 0; sm = P.sigma; }
+                if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+                R1 cjv;
+                cjv.x[0] = __ldg(P.cj + jh);
+                CCoef<HR, CC> cf{chs + tr * CC + tc + 1};
+                R1 out[4];
+                substep<1>(ut, jh, rm, rp, sm, sp, tc + 1, tc + 2, cf, cjv, P.tq_half, true, out, out);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) hs[c * HR * HC + tr * HC + tc] = out[c].x[0];
+            }
+        }
+    }
+    __syncthreads();
+    mbar_wait(&bar[1], 0);
+
+    CTile<HR, HC> ht{hs, j0 - 1};
+    // ---- full step, Eq. (14), radial Dirichlet rows, observer nodes
+    const int lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+    for (int k = 0; k < (TJ * TI + 255) / 256; ++k) {
+        int tr, tc;
+        if (TI == 32) { tr = warp + 8 * k; tc = lane; }
+        else { int idx = tid + k * 256; tr = idx / TI; tc = idx - tr * TI; }
+        int i = i0 + tc, j = j0 + tr;
+        if (tr >= TJ || i >= nr || j >= nt) continue;
+        R1 out[4];
+        if (i == 0 || i == nr - 1) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) out[c].x[0] = 0.0;
+        } else {
+            int rm = j - 1, rp = j + 1;
+            double sm = 1.0, sp = 1.0;
+            if (rm < 0) { rm = 0; sm = P.sigma; }
+            if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+            R1 bs[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) bs[c] = ut.get(c, j, tc + 2);
+            R1 cjv;
+            cjv.x[0] = __ldg(P.cj + j);
+            CCoef<TJ, TI> cf{cis + tr * TI + tc};
+            substep<1>(ht, j, rm, rp, sm, sp, tc, tc + 1, cf, cjv, P.tq_full, false, bs, out);
+        }
+        long g = (long)j * P.pitch + i;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) P.u_out[(long)c * P.plane + g] = out[c].x[0];
+        if (P.obs_raw != nullptr) {
+            int di = i - P.oi, dj = j - P.oj;
+            if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
+                long ks = *P.step_base + P.step_off;
+                if (ks < P.obs_cap) {
+                    double* o = P.obs_raw + ((ks * 4 + (dj * 2 + di)) * 4);
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) o[c] = out[c].x[0];
+                }
+            }
+        }
+    }
+}
+
+}  // namespace tk

@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -13,13 +14,18 @@
 #include "setup_kernels.cuh"
 #include "setup_math.cuh"
 #include "step_kernel.cuh"
+#include "step_kernel_tma.cuh"
 
 using namespace tk;
 
-#define CK(call)                                  \
-    do {                                          \
-        cudaError_t e_ = (call);                  \
-        if (e_ != cudaSuccess) return TEUK_ECUDA; \
+static int cuda_fail(cudaError_t e, const char* what, int line) {
+    if (getenv("TEUK_DEBUG")) fprintf(stderr, "[teuk] CUDA error %d (%s) at line %d: %s\n", (int)e, cudaGetErrorString(e), line, what);
+    return TEUK_ECUDA;
+}
+#define CK(call)                                                      \
+    do {                                                              \
+        cudaError_t e_ = (call);                                      \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call, __LINE__); \
     } while (0)
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -65,7 +71,10 @@ struct teuk_ctx {
     cudaStream_t stream;
     SetupConsts C;
     // options
-    int graph_steps = 32, opt_ti = 0, opt_tj = 0;
+    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1;
+    // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
+    bool use_tma = false;
+    CUtensorMap tm_state[2], tm_ch, tm_ci;
     // geometry
     int ti = 0, tj = 0, threads = 256;
     dim3 grid;
@@ -259,6 +268,8 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     } else if (!strcmp(key, "tile_j")) {
         if (v < 0 || v > 256) return TEUK_EINVAL;
         c->opt_tj = v;
+    } else if (!strcmp(key, "use_tma")) {
+        c->opt_tma = v != 0;
     } else if (!strcmp(key, "threads")) {
         if (v < 32 || v > 256 || (v % 32) != 0) return TEUK_EINVAL;
         c->threads = v;
@@ -292,7 +303,50 @@ static size_t smem_bytes(int L, int ti, int tj) {
     return (size_t)4 * L * ((size_t)(ti + 2) * (tj + 4) + (size_t)(ti + 1) * (tj + 2)) * sizeof(double);
 }
 
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 3-D tensor map over `planes` fp64 planes of n_theta rows x cols columns (row pitch `pitch`, plane stride `plane`)
+static bool make_map(CUtensorMap* tm, double* ptr, int cols, int n_theta, int planes, int pitch, long plane, int bx,
+                     int by, int bz) {
+    static EncodeTiledFn enc = nullptr;
+    if (!enc) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return false;
+        enc = (EncodeTiledFn)fn;
+    }
+    cuuint64_t dims[3] = {(cuuint64_t)cols, (cuuint64_t)n_theta, (cuuint64_t)planes};
+    cuuint64_t strides[2] = {(cuuint64_t)pitch * 8, (cuuint64_t)plane * 8};
+    cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz};
+    cuuint32_t es[3] = {1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, ptr, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int TI, int TJ> static bool setup_tma(teuk_ctx* c) {
+    using G = TmaGeom<TI, TJ>;
+    const Layout& y = c->lay;
+    bool ok = make_map(&c->tm_state[0], c->state(0), c->n_r, c->n_theta, 4, y.pitch, y.plane, G::UC, G::UR, 4) &&
+              make_map(&c->tm_state[1], c->state(1), c->n_r, c->n_theta, 4, y.pitch, y.plane, G::UC, G::UR, 4) &&
+              make_map(&c->tm_ch, c->dptr(y.coef_h), c->n_r - 1, c->n_theta, 8, y.pitch, y.plane, G::CC, G::HR, 8) &&
+              make_map(&c->tm_ci, c->dptr(y.coef_i), c->n_r, c->n_theta, 8, y.pitch, y.plane, TI, TJ, 8);
+    if (!ok) return false;
+    if (cudaFuncSetAttribute(step_kernel_f64_tma<TI, TJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::TOTAL) != cudaSuccess)
+        return false;
+    c->ti = TI; c->tj = TJ; c->smem = G::TOTAL; c->threads = 256;
+    c->grid = dim3((c->n_r + TI - 1) / TI, (c->n_theta + TJ - 1) / TJ);
+    return true;
+}
+
 static int choose_geometry(teuk_ctx* c) {
+    c->use_tma = false;
+    if (c->L == 1 && c->opt_tma && (c->opt_ti == 0 || c->opt_ti == 32) && (c->opt_tj == 0 || c->opt_tj == 8 || c->opt_tj == 16)) {
+        bool ok = (c->opt_tj == 8) ? setup_tma<32, 8>(c) : setup_tma<32, 16>(c);
+        cudaGetLastError();
+        if (ok) { c->use_tma = true; return TEUK_OK; }
+    }
     int ti = c->opt_ti, tj = c->opt_tj;
     if (ti == 0) ti = (c->L == 4) ? 16 : 32;
     if (tj == 0) {
@@ -330,7 +384,10 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
     P.obs_cap = c->obs_cap;
     P.step_off = step_off;
     P.oi = c->oi; P.oj = c->oj;
-    if (c->L == 1) step_kernel<1><<<c->grid, c->threads, c->smem, c->stream>>>(P);
+    if (c->use_tma) {
+        if (c->tj == 8) step_kernel_f64_tma<32, 8><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ch, c->tm_ci, P);
+        else step_kernel_f64_tma<32, 16><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ch, c->tm_ci, P);
+    } else if (c->L == 1) step_kernel<1><<<c->grid, c->threads, c->smem, c->stream>>>(P);
     else if (c->L == 2) step_kernel<2><<<c->grid, c->threads, c->smem, c->stream>>>(P);
     else step_kernel<4><<<c->grid, c->threads, c->smem, c->stream>>>(P);
     return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;

@@ -141,6 +141,27 @@ def test_tile_shapes_give_identical_results(teuk, ti, tj):
     assert np.array_equal(ref, got)
 
 
+@pytest.mark.parametrize("n_r,n_t", [(203, 13), (512, 16), (1000, 70), (40, 3)])
+def test_tma_kernel_matches_generic_kernel_fp64(teuk, n_r, n_t):
+    """the fp64 TMA kernel (default) and the generic kernel run the same arithmetic; compiler FMA contraction
+    may differ between the two instantiations, so compare to a few ulps, and both against the oracle"""
+    w = inputs.config(2).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0)
+    w = w.scaled(dt_override=inputs.stable_dt(w))
+    u0 = inputs.random_state(n_r, n_t, 1, seed=21)
+    outs = {}
+    for name, opts in (("tma16", {}), ("tma8", {"tile_j": 8}), ("generic", {"use_tma": 0})):
+        g = run_gpu(teuk, w, u0, 64, options=opts, observer=(10.3, 1.1))
+        outs[name] = (g.read(), g.observe(64), g.step_geometry())
+    assert outs["tma16"][2]["tile_j"] == 16 and outs["tma8"][2]["tile_j"] == 8
+    o = run_oracle(w, u0, 64, observer=(10.3, 1.1))
+    ref, sref = o.read(), o.observe(64)
+    for name, (u, ser, _) in outs.items():
+        assert max(oracle.rel_linf(u, ref).values()) <= TOL[1], name
+        assert max(series_err(ser, sref).values()) <= TOL[1], name
+    assert max(oracle.rel_linf(outs["tma16"][0], outs["generic"][0]).values()) <= 1e-14
+    assert np.array_equal(outs["tma16"][0], outs["tma8"][0])
+
+
 # ------------------------------------------------------------------------------- full-size configs (bench launch geometry)
 @pytest.mark.parametrize("cfg,steps_gpu,k", [(2, 300, 12), (3, 120, 8), (4, 100, 6)])
 def test_full_size_configs_windowed(teuk, cfg, steps_gpu, k):
