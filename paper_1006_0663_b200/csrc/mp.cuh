@@ -6,7 +6,7 @@
 //     reassociate it (nvcc's default -fmad=true stays on for the fp64 kernel);
 //   * all operations are BRANCH-FREE (the paper blames the QD library's branching and irregular memory
 //     access for its 1x "quadruple" result on Tesla): renormalisation is a fixed
-//     sequence of FastTwoSum passes without zero tests;
+//     sequence of TwoSum / FastTwoSum passes without zero tests;
 //   * limbs live in registers as x[0] (leading) .. x[L-1]; in memory every limb is its own plane.
 // Accuracy contract (checked by tests/test_device_arith.py against exact rationals): add/sub/mul
 // relative error <= 4 * 2^-104 (dd) and <= 16 * 2^-205 (qd) measured against max(|a|,|b|) for
@@ -117,14 +117,11 @@ MPX R1 div(const R1& a, const R1& b) { R1 r; r.x[0] = a.x[0] / b.x[0]; return r;
 
 // ------------------------------------------------------------------------------------- dd
 MPX R2 add(const R2& a, const R2& b) {
-    // TwoSum of the heads and of the tails, two FastTwoSum folds (error <= 3 * 2^-106 |a + b| when
-    // no cancellation; always <= 2^-105 (|a| + |b|))
-    double s, e, t, f;
+    // TwoSum of the heads, tails added in plain fp64, one FastTwoSum: 11 flops.  Absolute error
+    // <= 2^-105 (|a| + |b|) (the "sloppy" contract: relative to the operands, not to a cancelled sum).
+    double s, e;
     two_sum(a.x[0], b.x[0], s, e);
-    two_sum(a.x[1], b.x[1], t, f);
-    e = dadd(e, t);
-    fast_two_sum(s, e, s, e);
-    e = dadd(e, f);
+    e = dadd(e, dadd(a.x[1], b.x[1]));
     R2 r;
     fast_two_sum(s, e, r.x[0], r.x[1]);
     return r;
@@ -161,25 +158,33 @@ MPX R2 div(const R2& a, const R2& b) {
 }
 
 // ------------------------------------------------------------------------------------- qd
-// Bring five components of roughly decreasing order back to four non-overlapping limbs.  Fixed
-// sequence of error-free TwoSum passes (one bottom-up, two top-down) and a single rounded add at
-// the very end; no zero tests and no ordering assumptions (a zero intermediate just leaves a
-// harmless hole), so it is branch-free and loses nothing above order eps^4.
+// Renormalisation of five components into four limbs; two fixed, branch-free sequences:
+//  * renorm5: no ordering assumption (sums may have cancelled): an error-free bottom-up TwoSum pass, then
+//    one top-down TwoSum pass; the result is exact up to the single rounded add at the end and its limbs
+//    are ulp-non-overlapping (|x[k+1]| <= ulp(x[k])), which is all the other operations assume;
+//  * renorm4_ordered: for products, whose components are ordered by construction (|c[k+1]| <~ eps |c[k]|):
+//    FastTwoSum passes (3 flops each, half the dependency depth).
 MPX R4 renorm5(double c0, double c1, double c2, double c3, double c4) {
     double s, e, t0, t1, t2, t3, t4;
     two_sum(c3, c4, s, t4);
     two_sum(c2, s, s, t3);
     two_sum(c1, s, s, t2);
     two_sum(c0, s, t0, t1);
-    two_sum(t0, t1, t0, e);
-    two_sum(e, t2, t1, e);
-    two_sum(e, t3, t2, e);
-    two_sum(e, t4, t3, t4);
-    two_sum(t0, t1, t0, e);
-    two_sum(e, t2, t1, e);
-    two_sum(e, t3, t2, e);
     R4 r;
-    r.x[0] = t0; r.x[1] = t1; r.x[2] = t2; r.x[3] = dadd(e, t4);
+    r.x[0] = t0;
+    two_sum(t1, t2, r.x[1], e);
+    two_sum(e, t3, r.x[2], e);
+    r.x[3] = dadd(e, t4);
+    return r;
+}
+MPX R4 renorm4_ordered(double c0, double c1, double c2, double c3) {
+    double s, e, t1, t2, t3;
+    fast_two_sum(c2, c3, s, t3);
+    fast_two_sum(c1, s, s, t2);
+    R4 r;
+    fast_two_sum(c0, s, r.x[0], t1);
+    fast_two_sum(t1, t2, r.x[1], e);
+    fast_two_sum(e, t3, r.x[2], r.x[3]);
     return r;
 }
 
@@ -224,7 +229,7 @@ MPX R4 mul(const R4& a, const R4& b) {
     double t = dadd(dadd(q3, q4), dadd(q5, q0));
     double v = dadd(dadd(e1, e2), dadd(e3, dadd(e4, e5)));
     s3 = dadd(s3, dadd(t, v));
-    return renorm5(p0, p1, s2, s3, 0.0);
+    return renorm4_ordered(p0, p1, s2, s3);
 }
 
 MPX R4 mul_d(const R4& a, double d) {
@@ -236,7 +241,7 @@ MPX R4 mul_d(const R4& a, double d) {
     two_sum(q0, p1, p1, q0);              // order 1; q0 order 2
     three_sum(p2, q1, q0);                // order 2; q1 order 3, q0 order 4
     p3 = dadd(dadd(p3, q2), dadd(q1, q0));
-    return renorm5(p0, p1, p2, p3, 0.0);
+    return renorm4_ordered(p0, p1, p2, p3);
 }
 
 MPX R4 div(const R4& a, const R4& b) {

@@ -128,8 +128,10 @@ template <int L> struct SmemTile {
     }
 };
 
-template <int L>
-__global__ void __launch_bounds__(256) step_kernel(StepParams P) {
+// MAXT/MINB: launch bounds (register budget = 65536 / (MAXT * MINB)); the qd kernel is latency-bound at
+// 1 block x 8 warps, so variants trading registers for resident warps are instantiated and selectable.
+template <int L, int MAXT = 256, int MINB = 1>
+__global__ void __launch_bounds__(MAXT, MINB) step_kernel(StepParams P) {
     extern __shared__ double smem[];
     const int TI = P.ti, TJ = P.tj;
     const int UC = TI + 2, UR = TJ + 4, HC = TI + 1, HR = TJ + 2;

@@ -71,7 +71,7 @@ struct teuk_ctx {
     cudaStream_t stream;
     SetupConsts C;
     // options
-    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1;
+    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
     bool use_tma = false;
     CUtensorMap tm_state[2], tm_ch, tm_ci;
@@ -268,6 +268,9 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     } else if (!strcmp(key, "tile_j")) {
         if (v < 0 || v > 256) return TEUK_EINVAL;
         c->opt_tj = v;
+    } else if (!strcmp(key, "variant")) {
+        if (v < 0 || v > 2) return TEUK_EINVAL;
+        c->variant = v;
     } else if (!strcmp(key, "use_tma")) {
         c->opt_tma = v != 0;
     } else if (!strcmp(key, "threads")) {
@@ -340,6 +343,13 @@ template <int TI, int TJ> static bool setup_tma(teuk_ctx* c) {
     return true;
 }
 
+static const void* step_fn(const teuk_ctx* c) {
+    if (c->L == 1) return (const void*)step_kernel<1>;
+    if (c->L == 2) return c->variant == 0 ? (const void*)step_kernel<2, 256, 2> : c->variant == 1 ? (const void*)step_kernel<2, 128, 5> : (const void*)step_kernel<2, 128, 6>;
+    // qd: 128 threads x 3 blocks/SM (168 registers, a few spills) measured 1.9x faster than 256 x 1 (254 registers)
+    return c->variant == 0 ? (const void*)step_kernel<4, 128, 3> : c->variant == 1 ? (const void*)step_kernel<4, 256, 1> : (const void*)step_kernel<4, 128, 4>;
+}
+
 static int choose_geometry(teuk_ctx* c) {
     c->use_tma = false;
     if (c->L == 1 && c->opt_tma && (c->opt_ti == 0 || c->opt_ti == 32) && (c->opt_tj == 0 || c->opt_tj == 8 || c->opt_tj == 16)) {
@@ -361,9 +371,9 @@ static int choose_geometry(teuk_ctx* c) {
     c->ti = ti; c->tj = tj; c->smem = sm;
     c->grid = dim3((c->n_r + ti - 1) / ti, (c->n_theta + tj - 1) / tj);
     cudaError_t e = cudaSuccess;
-    if (c->L == 1) e = cudaFuncSetAttribute(step_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (c->L == 2) e = cudaFuncSetAttribute(step_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (c->L == 4) e = cudaFuncSetAttribute(step_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    const void* fn = step_fn(c);
+    c->threads = (c->L == 4) ? (c->variant == 1 ? 256 : 128) : (c->L == 2 && c->variant > 0 ? 128 : 256);
+    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     return e == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
 }
 
@@ -387,9 +397,10 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
     if (c->use_tma) {
         if (c->tj == 8) step_kernel_f64_tma<32, 8><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ch, c->tm_ci, P);
         else step_kernel_f64_tma<32, 16><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ch, c->tm_ci, P);
-    } else if (c->L == 1) step_kernel<1><<<c->grid, c->threads, c->smem, c->stream>>>(P);
-    else if (c->L == 2) step_kernel<2><<<c->grid, c->threads, c->smem, c->stream>>>(P);
-    else step_kernel<4><<<c->grid, c->threads, c->smem, c->stream>>>(P);
+    } else {
+        void* args[] = {&P};
+        if (cudaLaunchKernel(step_fn(c), c->grid, dim3(c->threads), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
+    }
     return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
 }
 
