@@ -35,6 +35,7 @@ def parse():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--no-extra", action="store_true", help="skip the dd/qd side measurements and the cpu baseline")
     ap.add_argument("--option", action="append", default=[], help="key=value passed to teuk_set_option")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE.json config 5: one JSON line per (N_r, N_theta, precision) cell")
     return ap.parse_args()
 
 
@@ -228,10 +229,41 @@ def load_traffic(name):
         return None
 
 
+def run_sweep(args):
+    """BASELINE.json config 5 (a = 0.99, s = -2, m = 2): updates/s and roofline fraction per cell.  fp64: HBM fraction
+    (192 B/update vs MEASURED_PEAKS hbm_gbs); dd/qd: FP64-pipe fraction = measured FP64 thread instructions per update
+    (ncu, profiles/r01b_step_kernels_ncu.md: 1345 dd, 13630 qd FP64 instructions per update, redundant halo work included) x updates/s / measured DFMA-chain peak."""
+    import torch
+    from paper_1006_0663_b200 import teuk
+    torch.cuda.set_device(0)
+    peak, _ = measured_peaks()
+    pipe = teuk.bench_fp64("dadd")
+    inst = {2: 1345.0, 4: 13630.0}
+    for L in (1, 2, 4):
+        for nr in (4096, 16384, 65536):
+            for nt in (32, 64, 256):
+                w = workload(f"sweep:{nr}x{nt}:{L}")
+                steps = {1: 1000, 2: 300, 4: 100}[L] if args.steps == 2000 else args.steps
+                ms, launches, geom, finite = time_device(torch, teuk, w, steps, 10, args.option)
+                ups = nr * nt * steps / (ms * 1e-3)
+                line = {"workload": w.name, "precision_limbs": L, "n_r": nr, "n_theta": nt, "steps": steps,
+                        "dt_over_dr": w.dt / w.dr, "updates_per_s": ups, "ms_per_step": ms / steps, "finite": finite,
+                        "geometry": geom}
+                if L == 1:
+                    line["roofline"] = {"bound": "hbm", "frac": ups * 192.0 / 1e9 / peak, "peak_gbs": peak,
+                                        "working_set_mib": 24 * nr * nt * 8 // 2 ** 20}
+                else:
+                    line["roofline"] = {"bound": "fp64 pipe", "frac": ups * inst[L] / pipe, "peak_inst_per_s": pipe,
+                                        "fp64_inst_per_update": inst[L]}
+                print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     import torch
     import torch.distributed as dist
     rank = int(os.environ.get("RANK", "0"))

@@ -128,91 +128,143 @@ template <int L> struct SmemTile {
     }
 };
 
-// MAXT/MINB: launch bounds (register budget = 65536 / (MAXT * MINB)); the qd kernel is latency-bound at
-// 1 block x 8 warps, so variants trading registers for resident warps are instantiated and selectable.
-template <int L, int MAXT = 256, int MINB = 1>
+template <int L> struct RegCoef {          // the 8 coefficients of one point, register resident
+    Real<L> c[8];
+    __device__ __forceinline__ const Real<L>& get(int q) const { return c[q]; }
+};
+template <int L>
+__device__ __forceinline__ void load_coef(RegCoef<L>& rc, const double* __restrict__ p, long stride, long idx) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) rc.c[q] = Ld<L>::g(p + (long)q * L * stride, stride, idx);
+}
+
+// Generic fused step kernel (all precisions; the default for dd and qd).
+//  * TI_/TJ_ > 0: compile-time tile (index arithmetic folds to constants); 0: run-time tile from P.ti/P.tj.
+//  * MAXT/MINB: launch bounds (register budget = 65536 / (MAXT * MINB)); the qd kernel is latency-bound at
+//    1 block x 8 warps, so shapes trading registers for resident warps are instantiated and selectable.
+//  * L <= 2: the coefficients of a thread's NEXT point are fetched into registers while it computes the current
+//    one, and the first set of each phase is requested before the preceding barrier (ncu on the first dd
+//    kernel: 48 % of stall cycles were long-scoreboard waits on exactly these loads).  qd has no registers to
+//    spare for that and is FP64-pipe bound anyway.
+template <int L, int TI_ = 0, int TJ_ = 0, int MAXT = 256, int MINB = 1>
 __global__ void __launch_bounds__(MAXT, MINB) step_kernel(StepParams P) {
     extern __shared__ double smem[];
-    const int TI = P.ti, TJ = P.tj;
+    const int TI = TI_ ? TI_ : P.ti, TJ = TJ_ ? TJ_ : P.tj;
     const int UC = TI + 2, UR = TJ + 4, HC = TI + 1, HR = TJ + 2;
     double* us = smem;                       // [4L][UR][UC]
     double* hs = smem + 4 * L * UR * UC;     // [4L][HR][HC]
     const int i0 = blockIdx.x * TI, j0 = blockIdx.y * TJ;
     const int iu0 = i0 - 1, ju0 = j0 - 2, jh0 = j0 - 1;
     const int nt = P.n_theta, nr = P.n_r;
-    const int tid = threadIdx.x, nth = blockDim.x;
+    const int tid = threadIdx.x, nth = MAXT;
+    constexpr bool PF = (L <= 2);
+
+    // work item -> tile coordinates; returns whether the item exists and lies inside the grid
+    auto item1 = [&](int idx, int& tc, int& tr, int& ih, int& jh) {
+        tr = idx / HC; tc = idx - tr * HC;
+        ih = iu0 + tc; jh = jh0 + tr;
+        return idx < HR * HC && ih >= 0 && ih <= nr - 2 && jh >= 0 && jh < nt;
+    };
+    auto item2 = [&](int idx, int& tc, int& tr, int& i, int& j) {
+        tr = idx / TI; tc = idx - tr * TI;
+        i = i0 + tc; j = j0 + tr;
+        return idx < TJ * TI && i < nr && j < nt;
+    };
+
+    RegCoef<L> cc;
+    int idx = tid, tc, tr, gi, gj;
+    bool v = item1(idx, tc, tr, gi, gj);
+    if (PF && v) load_coef(cc, P.coef_h, P.plane, (long)gj * P.pitch + gi);
 
     // ---- phase 0: stage the u^n tile (+1 column, +2 rows of halo); outside the grid -> 0
-    for (int idx = tid; idx < 4 * L * UR * UC; idx += nth) {
-        int tc = idx % UC, rest = idx / UC;
-        int tr = rest % UR, pl = rest / UR;
-        int gi = iu0 + tc, gj = ju0 + tr;
-        double v = 0.0;
-        if (gi >= 0 && gi < nr && gj >= 0 && gj < nt) v = __ldg(P.u_in + pl * P.plane + (long)gj * P.pitch + gi);
-        us[idx] = v;
+    for (int k = tid; k < 4 * L * UR * UC; k += nth) {
+        int c = k % UC, rest = k / UC;
+        int r = rest % UR, pl = rest / UR;
+        int ui = iu0 + c, uj = ju0 + r;
+        double val = 0.0;
+        if (ui >= 0 && ui < nr && uj >= 0 && uj < nt) val = __ldg(P.u_in + pl * P.plane + (long)uj * P.pitch + ui);
+        us[k] = val;
     }
     __syncthreads();
 
     SmemTile<L> ut{us, UR, UC, ju0};
     // ---- phase 1: half step, Eq. (13), at (ih + 1/2, jh) for the columns/rows the full step needs
-    for (int idx = tid; idx < HR * HC; idx += nth) {
-        int tc = idx % HC, tr = idx / HC;
-        int ih = iu0 + tc, jh = jh0 + tr;
-        if (ih < 0 || ih > nr - 2 || jh < 0 || jh >= nt) continue;
-        int rm = jh - 1, rp = jh + 1;
-        double sm = 1.0, sp = 1.0;
-        if (rm < 0) { rm = 0; sm = P.sigma; }
-        if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
-        Real<L> cjv = Ld<L>::g(P.cj, nt, jh);
-        Real<L> out[4];
-        GlobalCoef<L> cf{P.coef_h, P.plane, (long)jh * P.pitch + ih};
-        substep<L>(ut, jh, rm, rp, sm, sp, tc, tc + 1, cf, cjv, P.tq_half, true, out, out);
+    while (idx < HR * HC) {
+        int nidx = idx + nth, ntc, ntr, ngi, ngj;
+        bool nv = item1(nidx, ntc, ntr, ngi, ngj);
+        RegCoef<L> cn;
+        if (PF && nv) load_coef(cn, P.coef_h, P.plane, (long)ngj * P.pitch + ngi);
+        if (v) {
+            const int ih = gi, jh = gj;
+            if (!PF) load_coef(cc, P.coef_h, P.plane, (long)jh * P.pitch + ih);
+            int rm = jh - 1, rp = jh + 1;
+            double sm = 1.0, sp = 1.0;
+            if (rm < 0) { rm = 0; sm = P.sigma; }
+            if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+            Real<L> cjv = Ld<L>::g(P.cj, nt, jh);
+            Real<L> out[4];
+            substep<L>(ut, jh, rm, rp, sm, sp, tc, tc + 1, cc, cjv, P.tq_half, true, out, out);
 #pragma unroll
-        for (int c = 0; c < 4; ++c)
+            for (int c = 0; c < 4; ++c)
 #pragma unroll
-            for (int l = 0; l < L; ++l) hs[(c * L + l) * HR * HC + tr * HC + tc] = out[c].x[l];
+                for (int l = 0; l < L; ++l) hs[(c * L + l) * HR * HC + tr * HC + tc] = out[c].x[l];
+        }
+        if (PF) cc = cn;
+        idx = nidx; tc = ntc; tr = ntr; gi = ngi; gj = ngj; v = nv;
     }
+    // first full-step coefficient set: requested before the barrier
+    idx = tid;
+    v = item2(idx, tc, tr, gi, gj);
+    bool interior = v && gi != 0 && gi != nr - 1;
+    if (PF && interior) load_coef(cc, P.coef_i, P.plane, (long)gj * P.pitch + gi);
     __syncthreads();
 
     SmemTile<L> ht{hs, HR, HC, jh0};
     // ---- phase 2: full step, Eq. (14), + radial Dirichlet rows + observer nodes
-    for (int idx = tid; idx < TJ * TI; idx += nth) {
-        int tc = idx % TI, tr = idx / TI;
-        int i = i0 + tc, j = j0 + tr;
-        if (i >= nr || j >= nt) continue;
-        Real<L> out[4];
-        if (i == 0 || i == nr - 1) {
+    while (idx < TJ * TI) {
+        int nidx = idx + nth, ntc, ntr, ngi, ngj;
+        bool nv = item2(nidx, ntc, ntr, ngi, ngj);
+        bool ninterior = nv && ngi != 0 && ngi != nr - 1;
+        RegCoef<L> cn;
+        if (PF && ninterior) load_coef(cn, P.coef_i, P.plane, (long)ngj * P.pitch + ngi);
+        if (v) {
+            const int i = gi, j = gj;
+            Real<L> out[4];
+            if (!interior) {
 #pragma unroll
-            for (int c = 0; c < 4; ++c) out[c] = from_double<L>(0.0);
-        } else {
-            int rm = j - 1, rp = j + 1;
-            double sm = 1.0, sp = 1.0;
-            if (rm < 0) { rm = 0; sm = P.sigma; }
-            if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
-            Real<L> base[4];
+                for (int c = 0; c < 4; ++c) out[c] = from_double<L>(0.0);
+            } else {
+                if (!PF) load_coef(cc, P.coef_i, P.plane, (long)j * P.pitch + i);
+                int rm = j - 1, rp = j + 1;
+                double sm = 1.0, sp = 1.0;
+                if (rm < 0) { rm = 0; sm = P.sigma; }
+                if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+                Real<L> base[4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) base[c] = ut.get(c, j, tc + 1);
-            Real<L> cjv = Ld<L>::g(P.cj, nt, j);
-            // h columns: tile col tc <-> i - 1/2, tc + 1 <-> i + 1/2
-            GlobalCoef<L> cf{P.coef_i, P.plane, (long)j * P.pitch + i};
-            substep<L>(ht, j, rm, rp, sm, sp, tc, tc + 1, cf, cjv, P.tq_full, false, base, out);
-        }
-        long g = (long)j * P.pitch + i;
+                for (int c = 0; c < 4; ++c) base[c] = ut.get(c, j, tc + 1);
+                Real<L> cjv = Ld<L>::g(P.cj, nt, j);
+                // h columns: tile col tc <-> i - 1/2, tc + 1 <-> i + 1/2
+                substep<L>(ht, j, rm, rp, sm, sp, tc, tc + 1, cc, cjv, P.tq_full, false, base, out);
+            }
+            long g = (long)j * P.pitch + i;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) Ld<L>::st(P.u_out + (long)c * L * P.plane, P.plane, g, out[c]);
-        if (P.obs_raw != nullptr) {
-            int di = i - P.oi, dj = j - P.oj;
-            if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
-                long k = *P.step_base + P.step_off;
-                if (k < P.obs_cap) {
-                    double* o = P.obs_raw + ((k * 4 + (dj * 2 + di)) * 4) * L;
+            for (int c = 0; c < 4; ++c) Ld<L>::st(P.u_out + (long)c * L * P.plane, P.plane, g, out[c]);
+            if (P.obs_raw != nullptr) {
+                int di = i - P.oi, dj = j - P.oj;
+                if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
+                    long k = *P.step_base + P.step_off;
+                    if (k < P.obs_cap) {
+                        double* o = P.obs_raw + ((k * 4 + (dj * 2 + di)) * 4) * L;
 #pragma unroll
-                    for (int c = 0; c < 4; ++c)
+                        for (int c = 0; c < 4; ++c)
 #pragma unroll
-                        for (int l = 0; l < L; ++l) o[c * L + l] = out[c].x[l];
+                            for (int l = 0; l < L; ++l) o[c * L + l] = out[c].x[l];
+                    }
                 }
             }
         }
+        if (PF) cc = cn;
+        idx = nidx; tc = ntc; tr = ntr; gi = ngi; gj = ngj; v = nv; interior = ninterior;
     }
 }
 

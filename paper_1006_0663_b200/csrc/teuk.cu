@@ -273,9 +273,6 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
         c->variant = v;
     } else if (!strcmp(key, "use_tma")) {
         c->opt_tma = v != 0;
-    } else if (!strcmp(key, "threads")) {
-        if (v < 32 || v > 256 || (v % 32) != 0) return TEUK_EINVAL;
-        c->threads = v;
     } else {
         return TEUK_EINVAL;
     }
@@ -343,11 +340,23 @@ template <int TI, int TJ> static bool setup_tma(teuk_ctx* c) {
     return true;
 }
 
-static const void* step_fn(const teuk_ctx* c) {
-    if (c->L == 1) return (const void*)step_kernel<1>;
-    if (c->L == 2) return c->variant == 0 ? (const void*)step_kernel<2, 256, 2> : c->variant == 1 ? (const void*)step_kernel<2, 128, 5> : (const void*)step_kernel<2, 128, 6>;
+// instantiation table of the generic kernel: (precision, variant, tile) -> function and block size
+static const void* step_fn(const teuk_ctx* c, int* threads) {
+    *threads = 256;
+    if (c->L == 1) return (const void*)step_kernel<1, 0, 0, 256, 4>;
+    if (c->L == 2) {
+        if (c->variant == 1) { *threads = 128; return (const void*)step_kernel<2, 0, 0, 128, 5>; }
+        if (c->variant == 2) { *threads = 128; return (const void*)step_kernel<2, 0, 0, 128, 6>; }
+        if (c->ti == 32 && c->tj == 16) return (const void*)step_kernel<2, 32, 16, 256, 2>;
+        if (c->ti == 64 && c->tj == 8) return (const void*)step_kernel<2, 64, 8, 256, 2>;
+        return (const void*)step_kernel<2, 0, 0, 256, 2>;
+    }
     // qd: 128 threads x 3 blocks/SM (168 registers, a few spills) measured 1.9x faster than 256 x 1 (254 registers)
-    return c->variant == 0 ? (const void*)step_kernel<4, 128, 3> : c->variant == 1 ? (const void*)step_kernel<4, 256, 1> : (const void*)step_kernel<4, 128, 4>;
+    if (c->variant == 1) return (const void*)step_kernel<4, 0, 0, 256, 1>;
+    *threads = 128;
+    if (c->variant == 2) return (const void*)step_kernel<4, 0, 0, 128, 4>;
+    if (c->ti == 16 && c->tj == 8) return (const void*)step_kernel<4, 16, 8, 128, 3>;
+    return (const void*)step_kernel<4, 0, 0, 128, 3>;
 }
 
 static int choose_geometry(teuk_ctx* c) {
@@ -371,8 +380,7 @@ static int choose_geometry(teuk_ctx* c) {
     c->ti = ti; c->tj = tj; c->smem = sm;
     c->grid = dim3((c->n_r + ti - 1) / ti, (c->n_theta + tj - 1) / tj);
     cudaError_t e = cudaSuccess;
-    const void* fn = step_fn(c);
-    c->threads = (c->L == 4) ? (c->variant == 1 ? 256 : 128) : (c->L == 2 && c->variant > 0 ? 128 : 256);
+    const void* fn = step_fn(c, &c->threads);
     e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     return e == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
 }
@@ -399,7 +407,9 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         else step_kernel_f64_tma<32, 16><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ch, c->tm_ci, P);
     } else {
         void* args[] = {&P};
-        if (cudaLaunchKernel(step_fn(c), c->grid, dim3(c->threads), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
+        int threads = 256;
+        const void* fn = step_fn(c, &threads);
+        if (cudaLaunchKernel(fn, c->grid, dim3(threads), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
     }
     return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
 }
