@@ -282,16 +282,11 @@ def main():
     with ClockSampler(local) as cs:
         ms, launches, geom, finite = time_device(torch, teuk, w, args.steps, args.warmup, args.option, d)
     clocks = cs.summary()
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if d is not None:
-        d.all_reduce(t, op=dist.ReduceOp.MAX)                     # max over ranks; replicas only, no data-path collective
-    ms_max = float(t.item())
-    value = world * points * args.steps / (ms_max * 1e-3)
+    from paper_1006_0663_b200 import replicas
+    # max over ranks of the device time, updates summed over ranks; replicas only, no data-path collective
+    ms_max, _, value = replicas.aggregate(ms, float(points) * args.steps, d, device="cuda")
     e2e_dt, h2d, d2h = time_e2e(torch, teuk, w, args.steps, args.option)
-    te = torch.tensor([e2e_dt], dtype=torch.float64, device="cuda")
-    if d is not None:
-        d.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_val = world * points * args.steps / float(te.item())
+    _, _, e2e_val = replicas.aggregate(e2e_dt * 1e3, float(points) * args.steps, d, device="cuda")
     if rank != 0:
         if d is not None:
             d.destroy_process_group()
