@@ -292,7 +292,9 @@ def main():
             d.destroy_process_group()
         return
     peak, peak_src = measured_peaks()
-    alg_bytes = ALG_BYTES_PER_UPDATE[L] * points
+    recompute = any(o.replace(" ", "") == "coef_variant=1" for o in args.option)
+    bytes_per_update = 80.0 if recompute else ALG_BYTES_PER_UPDATE[L]     # H1b variant (b): state 64 B + two 1/Sigma planes 16 B
+    alg_bytes = bytes_per_update * points
     achieved = alg_bytes / (ms / args.steps * 1e-3) / 1e9
     line = {
         "metric": "Teukolsky grid-point updates/s", "value": value, "unit": "updates/s", "n_gpus": world,
@@ -311,8 +313,8 @@ def main():
                         "state once per K-step call divided by K"},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": load_traffic(f"{w.name}"), "peak_source": peak_src, "kernel": f"step_kernel<{L}>",
-                     "algorithmic_bytes_per_update": ALG_BYTES_PER_UPDATE[L]},
+                     "traffic": load_traffic(f"{w.name}"), "peak_source": peak_src, "kernel": "step_kernel_f64_rc" if recompute else ("step_kernel_f64_tma" if L == 1 else f"step_kernel<{L}>"),
+                     "algorithmic_bytes_per_update": bytes_per_update},
     }
     if not args.no_extra and world == 1:
         per = {}

@@ -40,7 +40,9 @@ int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double r
                 void *cuda_stream, teuk_ctx **out);
 
 /* Options, only before teuk_set_initial (else TEUK_ESTATE): "graph_steps" (even, >= 2; steps per
- * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic). */
+ * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic), "use_tma" (fp64: 1 = TMA
+ * kernel, default; 0 = generic kernel), "variant" (dd/qd launch shape 0..2), "coef_variant" (0 = precomputed
+ * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only). */
 int teuk_set_option(teuk_ctx *, const char *key, double value);
 
 /* Observer at a fixed location: bilinear interpolation in (r*, theta) from the four
@@ -81,6 +83,9 @@ const char *teuk_strerror(int code);
 /* Coefficient planes as the kernel uses them, double[8][L][n_theta][rows] (rows = n_r, or n_r-1 when
  * half != 0), UNFOLDED: b, alpha_R, alpha_I, gamma_R, gamma_I, W_R, W_I, kappa.  Host output. */
 int teuk_get_tables(teuk_ctx *, int half, double *host_out);
+/* FOLDED coefficient planes the step kernel multiplies with, double[8][n_theta][rows], fp64 handles only:
+ * coef_variant 0 = the stored planes, 1 = rebuilt from the semi-recompute tables by a kernel. */
+int teuk_get_folded(teuk_ctx *, int half, int coef_variant, double *host_out);
 /* r and r - r_+ at the 2 n_r - 1 integer/half points as quad-double limbs, double[2 n_r - 1][4] each. */
 int teuk_get_radial(teuk_ctx *, double *host_r, double *host_delta);
 /* One arithmetic operation of the multiprecision layer, limbs in/out (L = 2 or 4);

@@ -182,14 +182,64 @@ def theta_tables(n_theta):
         return sn, cs, to_limbs(dth)
 
 
+# ----------------------------------------------------------------------------- theta stencils
+def fd_weights(order):
+    """Centred finite-difference weights of accuracy `order` (2 or 10) on
+    2N+1 = order+1 equally spaced points, derived exactly in rationals from the Taylor conditions
+        sum_k w_k k^p = p! [p == derivative]   for p = 0..2N   (a Vandermonde system).
+    Returns (c, d): first-derivative weights c[k], k = 1..N (antisymmetric: w_{-k} = -c[k], in units 1/h) and
+    second-derivative weights d[k], k = 0..N (symmetric, in units 1/h^2), as fractions.Fraction."""
+    from fractions import Fraction
+    N = order // 2
+    pts = list(range(-N, N + 1))
+    n = len(pts)
+
+    def solve(deriv):
+        A = [[Fraction(x) ** p for x in pts] for p in range(n)]
+        rhs = [Fraction(0)] * n
+        f = 1
+        for q in range(2, deriv + 1):
+            f *= q
+        rhs[deriv] = Fraction(f)
+        # Gauss-Jordan in exact arithmetic
+        M = [row + [r] for row, r in zip(A, rhs)]
+        for col in range(n):
+            piv = next(r for r in range(col, n) if M[r][col] != 0)
+            M[col], M[piv] = M[piv], M[col]
+            pv = M[col][col]
+            M[col] = [v / pv for v in M[col]]
+            for r in range(n):
+                if r != col and M[r][col] != 0:
+                    fct = M[r][col]
+                    M[r] = [a - fct * b for a, b in zip(M[r], M[col])]
+        return [M[r][n] for r in range(n)]
+    w1, w2 = solve(1), solve(2)
+    c = [w1[N + k] for k in range(1, N + 1)]
+    d = [w2[N + k] for k in range(0, N + 1)]
+    assert all(w1[N - k] == -w1[N + k] for k in range(1, N + 1)) and w1[N] == 0
+    assert all(w2[N - k] == w2[N + k] for k in range(1, N + 1))
+    return c, d
+
+
+def fd_weight_limbs(order):
+    """the same weights as quad-double limbs: (c_limbs [N][4], d_limbs [N+1][4])"""
+    c, d = fd_weights(order)
+    with mp.workdps(MP_DPS):
+        cl = [to_limbs(mp.mpf(v.numerator) / mp.mpf(v.denominator)) for v in c]
+        dl = [to_limbs(mp.mpf(v.numerator) / mp.mpf(v.denominator)) for v in d]
+    return cl, dl
+
+
 # ----------------------------------------------------------------------------- Eqs. (13)-(14)
 class MPStepper:
     """Literal mpmath implementation of one Lax-Wendroff iteration on a tiny
     grid, every quantity (tables included) at `dps` digits.  Used by pin P9 (precision ladder)
     as the brute-force end of the ladder.  State u[f][i][j], f = Phi_R, Phi_I, Pi_R, Pi_I."""
 
-    def __init__(self, M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, dps=100):
+    def __init__(self, M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, dps=100, theta_order=2):
         self.dps = dps
+        self.theta_order = theta_order
+        self.wc, self.wd = fd_weights(theta_order)
         with mp.workdps(dps):
             self.n_r, self.n_t = n_r, n_theta
             self.M, self.a, self.s, self.m = mp.mpf(M), mp.mpf(a), s, m
@@ -219,11 +269,27 @@ class MPStepper:
                     self.u[f][0][j] = mp.mpf(0)
                     self.u[f][self.n_r - 1][j] = mp.mpf(0)
 
-    def _lam(self, col, j):
+    def _ghost(self, col, idx):
         nt = self.n_t
-        fm = col[j - 1] if j > 0 else self.sigma * col[0]
-        fp = col[j + 1] if j < nt - 1 else self.sigma * col[nt - 1]
-        return (fp + fm - 2 * col[j]) / self.dth ** 2 + self.cot[j] * (fp - fm) / (2 * self.dth)
+        if idx < 0:
+            return self.sigma * col[-idx - 1]
+        if idx >= nt:
+            return self.sigma * col[2 * nt - 1 - idx]
+        return col[idx]
+
+    def _lam(self, col, j):
+        if self.theta_order == 2:
+            fm, fp = self._ghost(col, j - 1), self._ghost(col, j + 1)
+            return (fp + fm - 2 * col[j]) / self.dth ** 2 + self.cot[j] * (fp - fm) / (2 * self.dth)
+        N = self.theta_order // 2
+        frac = lambda q: mp.mpf(q.numerator) / mp.mpf(q.denominator)
+        second = frac(self.wd[0]) * col[j]
+        first = mp.mpf(0)
+        for k in range(1, N + 1):
+            fp, fm = self._ghost(col, j + k), self._ghost(col, j - k)
+            second += frac(self.wd[k]) * (fp + fm)
+            first += frac(self.wc[k - 1]) * (fp - fm)
+        return second / self.dth ** 2 + self.cot[j] * first / self.dth
 
     def _substep(self, c, lo4, hi4, j, base4, tau):
         """shared algebra of Eqs. (13)/(14): lo4/hi4 = the two neighbour columns (per field),

@@ -42,7 +42,7 @@ def lib():
         dp = C.POINTER(C.c_double)
         _lib.oracle_create.argtypes = [C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
                                        C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, dp, dp, dp, dp, dp, dp,
-                                       C.POINTER(C.c_void_p)]
+                                       C.c_int, dp, dp, C.POINTER(C.c_void_p)]
         _lib.oracle_set_observer.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_long]
         _lib.oracle_set_initial.argtypes = [C.c_void_p, dp, C.c_int]
         _lib.oracle_step.argtypes = [C.c_void_p, C.c_long]
@@ -85,7 +85,8 @@ _table_cache: dict = {}
 class Oracle:
     """Plain CPU solver of PAPER.md §III.B; see teuk_oracle.cpp for the step-by-step citations."""
 
-    def __init__(self, M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision, i_lo=0, n_win=None):
+    def __init__(self, M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision, i_lo=0, n_win=None,
+                 theta_order=2):
         self.n_win = n_r - i_lo if n_win is None else n_win
         self.n_r, self.n_theta, self.L, self.i_lo = n_r, n_theta, precision, i_lo
         key = (float(M), float(a), float(rstar_min), float(rstar_max), n_r, i_lo, self.n_win)
@@ -93,18 +94,20 @@ class Oracle:
             _table_cache[key] = mp_ref.radial_tables(M, a, rstar_min, rstar_max, n_r, i_lo, self.n_win)
         r_l, d_l, dr_l = _table_cache[key]
         sn, cs, dth_l = mp_ref.theta_tables(n_theta)
-        self._keep = [np.ascontiguousarray(np.array(x, dtype=np.float64)) for x in (r_l, d_l, sn, cs, dr_l, dth_l)]
+        wc, wd = mp_ref.fd_weight_limbs(theta_order)
+        self._keep = [np.ascontiguousarray(np.array(x, dtype=np.float64)) for x in (r_l, d_l, sn, cs, dr_l, dth_l, wc, wd)]
         self.h = C.c_void_p()
+        k = [_dp(x) for x in self._keep]
         rc = lib().oracle_create(M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision, i_lo, self.n_win,
-                                 *[_dp(x) for x in self._keep], C.byref(self.h))
+                                 *k[:6], theta_order, k[6], k[7], C.byref(self.h))
         if rc != 0:
             self.h = None
             raise ValueError(f"oracle_create failed: {rc}")
 
     @classmethod
-    def from_workload(cls, w, precision=None, i_lo=0, n_win=None):
+    def from_workload(cls, w, precision=None, i_lo=0, n_win=None, theta_order=2):
         return cls(w.M, w.a, w.s, w.m, w.n_r, w.n_theta, w.rstar_min, w.rstar_max, w.dt,
-                   precision or w.precision, i_lo, n_win)
+                   precision or w.precision, i_lo, n_win, theta_order)
 
     def __del__(self):
         if getattr(self, "h", None):

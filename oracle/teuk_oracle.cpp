@@ -31,7 +31,7 @@ enum { OK = 0, EINVAL = -1, ESTATE = -4 };
 
 struct Params {
     double M, a, dt, rmin, rmax;
-    int s, m, n_r, n_theta, prec, i_lo, n_win;
+    int s, m, n_r, n_theta, prec, i_lo, n_win, theta_order;
 };
 
 // ---- O3: coefficients at one point, quad-double.  Same formulas as oracle/mp_ref.py::coefficients
@@ -80,7 +80,7 @@ struct Base {
     Params P;
     virtual ~Base() {}
     virtual int build(const double* r_tab, const double* d_tab, const double* sin_tab, const double* cos_tab,
-                      const double* dr_l, const double* dth_l) = 0;
+                      const double* dr_l, const double* dth_l, const double* wc_l, const double* wd_l) = 0;
     virtual int set_observer(double ro, double to, long cap) = 0;
     virtual int set_initial(const double* planes, int limbs_in) = 0;
     virtual int step(long n) = 0;
@@ -98,7 +98,8 @@ struct Solver : Base {
     struct C { T b, aR, aI, gR, gI, WR, WI, k; };
     std::vector<C> ci, ch;                // [i*n_theta + j]; ch has n_win-1 rows
     std::vector<T> cot;
-    T inv_dr, inv_dth2, inv_2dth, dt, half_dt;
+    T inv_dr, inv_dth2, inv_2dth, inv_dth, dt, half_dt;
+    std::vector<T> wc, wd;                // theta stencil weights (first derivative k = 1..N, second k = 0..N)
     Q dr_q, dth_q;
     int sigma;
     std::vector<T> u[4], un[4], h[4];     // [i*n_theta + j]
@@ -110,7 +111,7 @@ struct Solver : Base {
     std::vector<T> series;                // [sample][4]
 
     int build(const double* r_tab, const double* d_tab, const double* sin_tab, const double* cos_tab,
-              const double* dr_l, const double* dth_l) override {
+              const double* dr_l, const double* dth_l, const double* wc_l, const double* wd_l) override {
         const int nw = P.n_win, nt = P.n_theta;
         Q M(P.M), a(P.a);
         Q rpm = sqrt(M * M - a * a);
@@ -121,6 +122,11 @@ struct Solver : Base {
         inv_dr = narrow<T>(one / dr_q);
         inv_dth2 = narrow<T>(one / (dth_q * dth_q));
         inv_2dth = narrow<T>(one / (dth_q + dth_q));
+        inv_dth = narrow<T>(one / dth_q);
+        const int N = P.theta_order / 2;
+        wc.resize(N); wd.resize(N + 1);
+        for (int k = 0; k < N; ++k) wc[k] = narrow<T>(Q::from_limbs(wc_l + 4 * k, 4));
+        for (int k = 0; k <= N; ++k) wd[k] = narrow<T>(Q::from_limbs(wd_l + 4 * k, 4));
         dt = T(P.dt);
         half_dt = half_of<T>(dt);
         sigma = (std::abs(P.m) % 2 == 0) ? 1 : -1;
@@ -190,15 +196,34 @@ struct Solver : Base {
         return OK;
     }
 
-    // Lambda_j[f] = ((f_{j+1} + f_{j-1}) - 2 f_j)/dtheta^2 + cot(theta_j) (f_{j+1} - f_{j-1})/(2 dtheta)
-    // second-order centred differences with the polar ghosts of PAPER.md:112 (A9, A12).
-    T lam(const T* f, int j) const {
+    // polar ghosts (cell-centred grid, reading A9): f_{-k} = sigma f_{k-1}, f_{N-1+k} = sigma f_{N-k}
+    T ghost(const T* f, int idx) const {
         const int nt = P.n_theta;
-        T fm = (j > 0) ? f[j - 1] : (sigma > 0 ? f[0] : -f[0]);
-        T fp = (j < nt - 1) ? f[j + 1] : (sigma > 0 ? f[nt - 1] : -f[nt - 1]);
-        T second = ((fp + fm) - (f[j] + f[j])) * inv_dth2;
-        T first = cot[j] * ((fp - fm) * inv_2dth);
-        return second + first;
+        if (idx < 0) return sigma > 0 ? f[-idx - 1] : -f[-idx - 1];
+        if (idx >= nt) return sigma > 0 ? f[2 * nt - 1 - idx] : -f[2 * nt - 1 - idx];
+        return f[idx];
+    }
+    // theta_order 2:
+    //   Lambda_j[f] = ((f_{j+1} + f_{j-1}) - 2 f_j)/dtheta^2 + cot(theta_j) (f_{j+1} - f_{j-1})/(2 dtheta)
+    // theta_order 10 ("10th-order accurate" angular operator; 11-point centred stencils whose weights
+    // come from oracle/mp_ref.py::fd_weights):
+    //   Lambda_j[f] = (d_0 f_j + sum_k d_k (f_{j+k} + f_{j-k}))/dtheta^2 + cot(theta_j) (sum_k c_k (f_{j+k} - f_{j-k}))/dtheta
+    T lam(const T* f, int j) const {
+        if (P.theta_order == 2) {
+            T fm = ghost(f, j - 1), fp = ghost(f, j + 1);
+            T second = ((fp + fm) - (f[j] + f[j])) * inv_dth2;
+            T first = cot[j] * ((fp - fm) * inv_2dth);
+            return second + first;
+        }
+        const int N = P.theta_order / 2;
+        T s2 = wd[0] * f[j];
+        T s1 = T(0.0);
+        for (int k = 1; k <= N; ++k) {
+            T fp = ghost(f, j + k), fm = ghost(f, j - k);
+            s2 = s2 + wd[k] * (fp + fm);
+            s1 = s1 + wc[k - 1] * (fp - fm);
+        }
+        return s2 * inv_dth2 + cot[j] * (s1 * inv_dth);
     }
 
     // one sub-step source + update at a point; v = (mean fields), d = (differences)/dr*, lamR/I = Lambda[mean Phi]
@@ -379,16 +404,18 @@ extern "C" {
 
 int oracle_create(double M, double a, int s, int m, int n_r, int n_theta, double rmin, double rmax, double dt,
                   int precision, int i_lo, int n_win, const double* r_tab, const double* d_tab, const double* sin_tab,
-                  const double* cos_tab, const double* dr_l, const double* dth_l, void** out) {
+                  const double* cos_tab, const double* dr_l, const double* dth_l, int theta_order, const double* wc_l,
+                  const double* wd_l, void** out) {
     if (!(M > 0) || !(std::fabs(a) < M) || n_r < 3 || n_theta < 2 || !(dt > 0) || !(rmin < rmax) || !out) return EINVAL;
+    if ((theta_order != 2 && theta_order != 10) || n_theta < theta_order / 2) return EINVAL;
     if (i_lo < 0 || n_win < 3 || i_lo + n_win > n_r) return EINVAL;
     Base* b = nullptr;
     if (precision == 1) b = new Solver<double>();
     else if (precision == 2) b = new Solver<MP<2>>();
     else if (precision == 4) b = new Solver<MP<4>>();
     else return EINVAL;
-    b->P = Params{M, a, dt, rmin, rmax, s, m, n_r, n_theta, precision, i_lo, n_win};
-    int rc = b->build(r_tab, d_tab, sin_tab, cos_tab, dr_l, dth_l);
+    b->P = Params{M, a, dt, rmin, rmax, s, m, n_r, n_theta, precision, i_lo, n_win, theta_order};
+    int rc = b->build(r_tab, d_tab, sin_tab, cos_tab, dr_l, dth_l, wc_l, wd_l);
     if (rc != OK) { delete b; return rc; }
     *out = b;
     return OK;

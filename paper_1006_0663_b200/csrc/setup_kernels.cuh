@@ -147,3 +147,89 @@ __global__ void coef_kernel(SetupConsts C, const double* __restrict__ r_tab, con
 }
 
 }  // namespace tk
+
+namespace tk {
+
+// ---------------------------------------------------------------------------------------------------------------
+// Semi-recompute coefficient supply (variant (b); fp64 only).  Every coefficient of §3 is
+// q^k x (function of r) x (function of theta) with q = 1/Sigma^2, so instead of 16 two-dimensional planes the step
+// kernel reads ONE plane per point family (isig = 1/Sigma) plus 16 one-dimensional r-tables and 3 theta-tables:
+//   c0 = T0 isig                      c1 = T1 q                     c2 = (T2a + T2b cos) q
+//   c3 = q (T3a isig + T3b - q sin^2 T3c)                           c4 = q ((T4a + T4b cos) isig + T4c)
+//   c5 = q (T5a Tth + T5b)            c6 = q T6                     c7 = q T7,          q = isig^2,
+// Tth = (m + s cos)^2 / sin^2 - s.  HBM traffic: 64 B of state + 16 B of isig per update instead of 192 B.
+// Table order in memory: R-family f (0: integer points, tau = dt; 1: half points, tau = dt/2), table t = 0..15:
+//   T0 T1 T2a T2b T3a T3b T3c T4a T4b T4c T5a T5b T6 T7 (14 used, 2 spare), each `pitch` doubles.
+constexpr int RC_NT = 16;
+
+__global__ void rtab_kernel(SetupConsts C, const double* __restrict__ r_tab, const double* __restrict__ d_tab,
+                            double* __restrict__ rt) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= 2 * C.n_r - 1) return;
+    const int fam = k & 1, col = k >> 1;
+    R4 r, dl;
+#pragma unroll
+    for (int l = 0; l < 4; ++l) { r.x[l] = r_tab[4 * k + l]; dl.x[l] = d_tab[4 * k + l]; }
+    const R4 M = C.M, a = C.a;
+    const double s = (double)C.s, m = (double)C.m;
+    R4 r2 = mul(r, r), a2 = mul(a, a);
+    R4 R = add(r2, a2);
+    R4 Dl = mul(dl, add(dl, C.rpm));
+    R4 rmM = sub(r, M), rD = mul(r, Dl);
+    R4 AR = mul_d(sub(rD, mul(M, sub(r2, a2))), 2.0 * s);
+    R4 AI0 = mul_d(mul(mul(M, a), r), 4.0 * m);
+    R4 AI1 = mul_d(mul(a, Dl), 2.0 * s);
+    R4 CR = add(scale2(rD, 2.0), mul_d(mul(rmM, R), 2.0 * s));
+    R4 CI = mul_d(mul(a, R), 2.0 * m);
+    R4 DoR = div(Dl, R);
+    R4 g = mul_d(div(DoR, r), 3.0);
+    R4 gnum = sub(mul(scale2(rmM, 2.0), mul(r, R)), mul(Dl, add(mul_d(r2, 3.0), a2)));
+    R4 RR = mul(R, R);
+    R4 gst = mul_d(div(mul(DoR, gnum), mul(r2, RR)), 3.0);
+    R4 BR = add(mul(scale2(RR, 2.0), g), CR);
+    R4 BB = mul(mul(a2, Dl), sub(mul(R, rmM), scale2(rD, 2.0)));
+    R4 WR0 = neg(add(mul(RR, add(gst, mul(g, g))), mul(CR, g)));
+    R4 WIr = neg(add(mul_d(mul(a, rmM), 4.0 * m * s), mul(CI, g)));
+    R4 tau = fam ? C.tau_h : C.tau_f;
+    R4 tdr = div(tau, C.dr), th2 = scale2(tau, 0.5);
+    R4 tk = div(th2, mul(C.dth, C.dth));
+    R4 T[RC_NT];
+    T[0] = mul(tdr, R);
+    T[1] = mul(th2, AR);
+    T[2] = mul(th2, AI0);
+    T[3] = mul(th2, AI1);
+    T[4] = mul(tdr, mul(AR, R));
+    T[5] = mul(tdr, BR);
+    T[6] = mul(tdr, BB);
+    T[7] = mul(tdr, mul(AI0, R));
+    T[8] = mul(tdr, mul(AI1, R));
+    T[9] = mul(tdr, CI);
+    T[10] = mul(th2, Dl);
+    T[11] = mul(th2, WR0);
+    T[12] = mul(th2, WIr);
+    T[13] = mul(tk, Dl);
+    T[14] = RR;                       // spare slots keep R^2 and a^2 Delta (used by isig_kernel's checks / debugging)
+    T[15] = mul(a2, Dl);
+#pragma unroll
+    for (int t = 0; t < RC_NT; ++t) rt[((long)fam * RC_NT + t) * C.pitch + col] = T[t].x[0];
+}
+
+// isig = 1/Sigma at every point of both families, evaluated in quad-double, rounded to fp64.
+__global__ void isig_kernel(SetupConsts C, const double* __restrict__ r_tab, const double* __restrict__ d_tab,
+                            const double* __restrict__ sin_tab, int half, double* __restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    int cols = half ? C.n_r - 1 : C.n_r;
+    if (i >= cols) return;
+    int k = 2 * i + half;
+    R4 r, dl, sn;
+#pragma unroll
+    for (int l = 0; l < 4; ++l) { r.x[l] = r_tab[4 * k + l]; dl.x[l] = d_tab[4 * k + l]; sn.x[l] = sin_tab[4 * j + l]; }
+    R4 a2 = mul(C.a, C.a);
+    R4 R = add(mul(r, r), a2);
+    R4 Dl = mul(dl, add(dl, C.rpm));
+    R4 Sig2 = sub(mul(R, R), mul(mul(a2, Dl), mul(sn, sn)));
+    R4 is = div(from_double<4>(1.0), msqrt(Sig2));
+    out[(long)j * C.pitch + i] = is.x[0];
+}
+
+}  // namespace tk

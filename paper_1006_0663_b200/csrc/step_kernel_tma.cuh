@@ -180,4 +180,166 @@ __global__ void __launch_bounds__(256) step_kernel_f64_tma(const __grid_constant
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// fp64 step kernel, SEMI-RECOMPUTE coefficient supply (H1b variant (b), see setup_kernels.cuh): same phases and
+// the same substep<1> arithmetic as step_kernel_f64_tma, but the 16 coefficient planes are replaced by one
+// isig = 1/Sigma plane per point family plus 1-D tables, and the 8 folded coefficients of a point are rebuilt in
+// registers (17 extra flops per sub-step).  TMA loads per block: u tile, isig tile (half points), isig tile
+// (integer points), r-table slab (half points, 16 x (TI+2)), r-table slab (integer points, 16 x TI).
+struct RcParams {
+    const double* th;      // [3][n_theta]: sin^2, cos, Tth = (m + s cos)^2 / sin^2 - s
+};
+
+template <int TI, int TJ> struct RcGeom {
+    static constexpr int UC = TI + 4, UR = TJ + 4, HC = TI + 1, HR = TJ + 2, CC = TI + 2, NT = 16;
+    static constexpr int a128(int v) { return (v + 127) / 128 * 128; }
+    static constexpr int US_B = a128(4 * UR * UC * 8);
+    static constexpr int ISH_B = a128(HR * CC * 8);
+    static constexpr int ISI_B = a128(TJ * TI * 8);
+    static constexpr int RTH_B = a128(NT * CC * 8);
+    static constexpr int RTI_B = a128(NT * TI * 8);
+    static constexpr int HS_B = a128(4 * HR * HC * 8);
+    static constexpr int TOTAL = US_B + ISH_B + ISI_B + RTH_B + RTI_B + HS_B + 128;
+};
+
+struct RcCoef {
+    double c[8];
+    __device__ __forceinline__ R1 get(int q) const { R1 r; r.x[0] = c[q]; return r; }
+};
+// rt: pointer to this point's column in the r-table slab, consecutive tables `stride` apart
+__device__ __forceinline__ void rc_eval(RcCoef& o, double isig, const double* rt, int stride, double s2, double cs,
+                                        double tth) {
+    const double q = isig * isig;
+    o.c[0] = rt[0] * isig;
+    o.c[1] = rt[1 * stride] * q;
+    o.c[2] = fma(rt[3 * stride], cs, rt[2 * stride]) * q;
+    o.c[3] = q * fma(-(q * s2), rt[6 * stride], fma(rt[4 * stride], isig, rt[5 * stride]));
+    o.c[4] = q * fma(fma(rt[8 * stride], cs, rt[7 * stride]), isig, rt[9 * stride]);
+    o.c[5] = q * fma(rt[10 * stride], tth, rt[11 * stride]);
+    o.c[6] = q * rt[12 * stride];
+    o.c[7] = q * rt[13 * stride];
+}
+
+template <int TI, int TJ>
+__global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant__ CUtensorMap tm_u,
+                                                         const __grid_constant__ CUtensorMap tm_ish,
+                                                         const __grid_constant__ CUtensorMap tm_isi,
+                                                         const __grid_constant__ CUtensorMap tm_rth,
+                                                         const __grid_constant__ CUtensorMap tm_rti, StepParams P,
+                                                         RcParams Q) {
+    using G = RcGeom<TI, TJ>;
+    constexpr int UC = G::UC, UR = G::UR, HC = G::HC, HR = G::HR, CC = G::CC, NT = G::NT;
+    extern __shared__ __align__(128) unsigned char raw[];
+    __shared__ __align__(8) uint64_t bar[2];
+    unsigned char* base = (unsigned char*)(((uintptr_t)raw + 127) & ~(uintptr_t)127);
+    double* us = (double*)base;
+    double* ish = (double*)(base + G::US_B);
+    double* isi = (double*)(base + G::US_B + G::ISH_B);
+    double* rth = (double*)(base + G::US_B + G::ISH_B + G::ISI_B);
+    double* rti = (double*)(base + G::US_B + G::ISH_B + G::ISI_B + G::RTH_B);
+    double* hs = (double*)(base + G::US_B + G::ISH_B + G::ISI_B + G::RTH_B + G::RTI_B);
+    const int i0 = blockIdx.x * TI, j0 = blockIdx.y * TJ;
+    const int nt = P.n_theta, nr = P.n_r;
+    const int tid = threadIdx.x;
+
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&bar[0], 4 * UR * UC * 8 + HR * CC * 8 + NT * CC * 8);
+        tma_load_3d(us, &tm_u, i0 - 2, j0 - 2, 0, &bar[0]);
+        tma_load_3d(ish, &tm_ish, i0 - 2, j0 - 1, 0, &bar[0]);
+        tma_load_3d(rth, &tm_rth, i0 - 2, 0, 0, &bar[0]);
+        mbar_expect_tx(&bar[1], TJ * TI * 8 + NT * TI * 8);
+        tma_load_3d(isi, &tm_isi, i0, j0, 0, &bar[1]);
+        tma_load_3d(rti, &tm_rti, i0, 0, 0, &bar[1]);
+    }
+    mbar_wait(&bar[0], 0);
+
+    CTile<UR, UC> ut{us, j0 - 2};
+#pragma unroll
+    for (int k = 0; k < (HR * HC + 255) / 256; ++k) {
+        int idx = tid + k * 256;
+        if (idx < HR * HC) {
+            int tr = idx / HC, tc = idx - tr * HC;
+            int ih = i0 - 1 + tc, jh = j0 - 1 + tr;
+            if (ih >= 0 && ih <= nr - 2 && jh >= 0 && jh < nt) {
+                int rm = jh - 1, rp = jh + 1;
+                double sm = 1.0, sp = 1.0;
+                if (rm < 0) { rm = 0; sm = P.sigma; }
+                if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+                R1 cjv;
+                cjv.x[0] = __ldg(P.cj + jh);
+                RcCoef cf;
+                rc_eval(cf, ish[tr * CC + tc + 1], rth + tc + 1, CC, __ldg(Q.th + jh), __ldg(Q.th + nt + jh),
+                        __ldg(Q.th + 2 * nt + jh));
+                R1 out[4];
+                substep<1>(ut, jh, rm, rp, sm, sp, tc + 1, tc + 2, cf, cjv, P.tq_half, true, out, out);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) hs[c * HR * HC + tr * HC + tc] = out[c].x[0];
+            }
+        }
+    }
+    __syncthreads();
+    mbar_wait(&bar[1], 0);
+
+    CTile<HR, HC> ht{hs, j0 - 1};
+    const int lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+    for (int k = 0; k < (TJ * TI + 255) / 256; ++k) {
+        int tr, tc;
+        if (TI == 32) { tr = warp + 8 * k; tc = lane; }
+        else { int idx = tid + k * 256; tr = idx / TI; tc = idx - tr * TI; }
+        int i = i0 + tc, j = j0 + tr;
+        if (tr >= TJ || i >= nr || j >= nt) continue;
+        R1 out[4];
+        if (i == 0 || i == nr - 1) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) out[c].x[0] = 0.0;
+        } else {
+            int rm = j - 1, rp = j + 1;
+            double sm = 1.0, sp = 1.0;
+            if (rm < 0) { rm = 0; sm = P.sigma; }
+            if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+            R1 bs[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) bs[c] = ut.get(c, j, tc + 2);
+            R1 cjv;
+            cjv.x[0] = __ldg(P.cj + j);
+            RcCoef cf;
+            rc_eval(cf, isi[tr * TI + tc], rti + tc, TI, __ldg(Q.th + j), __ldg(Q.th + nt + j), __ldg(Q.th + 2 * nt + j));
+            substep<1>(ht, j, rm, rp, sm, sp, tc, tc + 1, cf, cjv, P.tq_full, false, bs, out);
+        }
+        long g = (long)j * P.pitch + i;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) P.u_out[(long)c * P.plane + g] = out[c].x[0];
+        if (P.obs_raw != nullptr) {
+            int di = i - P.oi, dj = j - P.oj;
+            if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
+                long ks = *P.step_base + P.step_off;
+                if (ks < P.obs_cap) {
+                    double* o = P.obs_raw + ((ks * 4 + (dj * 2 + di)) * 4);
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) o[c] = out[c].x[0];
+                }
+            }
+        }
+    }
+}
+
+// test hook: recomputed folded coefficients of one family written as 8 planes [n_theta][pitch]
+__global__ void rc_tables_kernel(const double* __restrict__ isig, const double* __restrict__ rt, const double* __restrict__ th,
+                                 int cols, int n_theta, int pitch, long plane, double* __restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= cols) return;
+    RcCoef cf;
+    rc_eval(cf, isig[(long)j * pitch + i], rt + i, pitch, th[j], th[n_theta + j], th[2 * n_theta + j]);
+    for (int q = 0; q < 8; ++q) out[q * plane + (long)j * pitch + i] = cf.c[q];
+}
+
 }  // namespace tk

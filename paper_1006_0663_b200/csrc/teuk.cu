@@ -33,7 +33,7 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 struct Layout {
     int pitch;
     long plane;
-    size_t state_a, state_b, coef_i, coef_h, cj, r_tab, d_tab, sin_tab, cos_tab, obs_raw, obs_out, scalars, total;
+    size_t state_a, state_b, coef_i, coef_h, cj, r_tab, d_tab, sin_tab, cos_tab, obs_raw, obs_out, scalars, rc_rt, rc_isig, rc_th, total;
 };
 
 static Layout make_layout(int n_r, int n_theta, int L, long cap) {
@@ -58,6 +58,10 @@ static Layout make_layout(int n_r, int n_theta, int L, long cap) {
     y.obs_raw = take((size_t)(cap > 0 ? cap : 1) * 16 * L);
     y.obs_out = take((size_t)(cap > 0 ? cap : 1) * 4 * L);
     y.scalars = take(8);
+    // semi-recompute supply (fp64 only): r-tables [2][16][pitch], isig planes [2][n_theta][pitch], theta tables [3][n_theta]
+    y.rc_rt = take(L == 1 ? (size_t)2 * RC_NT * y.pitch : 1);
+    y.rc_isig = take(L == 1 ? (size_t)2 * y.plane : 1);
+    y.rc_th = take(L == 1 ? (size_t)3 * n_theta : 1);
     y.total = off;
     return y;
 }
@@ -71,10 +75,10 @@ struct teuk_ctx {
     cudaStream_t stream;
     SetupConsts C;
     // options
-    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0;
+    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
-    bool use_tma = false;
-    CUtensorMap tm_state[2], tm_ch, tm_ci;
+    bool use_tma = false, use_rc = false;
+    CUtensorMap tm_state[2], tm_ch, tm_ci, tm_ish, tm_isi, tm_rth, tm_rti;
     // geometry
     int ti = 0, tj = 0, threads = 256;
     dim3 grid;
@@ -248,6 +252,29 @@ extern "C" int teuk_create(double M, double a, int s, int m, int n_r, int n_thet
     radial_kernel<<<(npts + 63) / 64, 64, 0, c->stream>>>(C, c->dptr(lay.r_tab), c->dptr(lay.d_tab));
     c->launches++;
     if (cudaGetLastError() != cudaSuccess) return fail(TEUK_ECUDA);
+    if (precision == 1) {
+        // semi-recompute supply: theta tables on the host in quad-double, r-tables and isig planes on the device
+        std::vector<double> th((size_t)3 * n_theta);
+        for (int j = 0; j < n_theta; ++j) {
+            R4 sj, cj;
+            for (int l = 0; l < 4; ++l) { sj.x[l] = sn[4 * j + l]; cj.x[l] = cs[4 * j + l]; }
+            R4 s2 = mul(sj, sj);
+            R4 mc = add(from_double<4>((double)m), mul_d(cj, (double)s));
+            R4 tth = sub(div(mul(mc, mc), s2), from_double<4>((double)s));
+            th[j] = s2.x[0]; th[n_theta + j] = cj.x[0]; th[2 * n_theta + j] = tth.x[0];
+        }
+        if (cudaMemcpyAsync(c->dptr(lay.rc_th), th.data(), th.size() * 8, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+            cudaStreamSynchronize(c->stream) != cudaSuccess)
+            return fail(TEUK_ECUDA);
+        rtab_kernel<<<(npts + 63) / 64, 64, 0, c->stream>>>(C, c->dptr(lay.r_tab), c->dptr(lay.d_tab), c->dptr(lay.rc_rt));
+        for (int half = 0; half < 2; ++half) {
+            int cols = half ? n_r - 1 : n_r;
+            isig_kernel<<<dim3((cols + 127) / 128, n_theta), 128, 0, c->stream>>>(
+                C, c->dptr(lay.r_tab), c->dptr(lay.d_tab), c->dptr(lay.sin_tab), half, c->dptr(lay.rc_isig) + (size_t)half * lay.plane);
+        }
+        c->launches += 3;
+        if (cudaGetLastError() != cudaSuccess) return fail(TEUK_ECUDA);
+    }
     if ((rc = launch_coef_any(c, 0, 1, c->dptr(lay.coef_i))) != TEUK_OK) return fail(rc);
     if ((rc = launch_coef_any(c, 1, 1, c->dptr(lay.coef_h))) != TEUK_OK) return fail(rc);
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) return fail(TEUK_ECUDA);
@@ -268,6 +295,9 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     } else if (!strcmp(key, "tile_j")) {
         if (v < 0 || v > 256) return TEUK_EINVAL;
         c->opt_tj = v;
+    } else if (!strcmp(key, "coef_variant")) {
+        if (v < 0 || v > 1 || (v == 1 && c->L != 1)) return TEUK_EINVAL;
+        c->coef_variant = v;
     } else if (!strcmp(key, "variant")) {
         if (v < 0 || v > 2) return TEUK_EINVAL;
         c->variant = v;
@@ -359,8 +389,35 @@ static const void* step_fn(const teuk_ctx* c, int* threads) {
     return (const void*)step_kernel<4, 0, 0, 128, 3>;
 }
 
+template <int TI, int TJ> static bool setup_rc(teuk_ctx* c) {
+    using G = RcGeom<TI, TJ>;
+    const Layout& y = c->lay;
+    double* is0 = c->dptr(y.rc_isig);
+    double* rt0 = c->dptr(y.rc_rt);
+    bool ok = make_map(&c->tm_state[0], c->state(0), c->n_r, c->n_theta, 4, y.pitch, y.plane, G::UC, G::UR, 4) &&
+              make_map(&c->tm_state[1], c->state(1), c->n_r, c->n_theta, 4, y.pitch, y.plane, G::UC, G::UR, 4) &&
+              make_map(&c->tm_isi, is0, c->n_r, c->n_theta, 1, y.pitch, y.plane, TI, TJ, 1) &&
+              make_map(&c->tm_ish, is0 + y.plane, c->n_r - 1, c->n_theta, 1, y.pitch, y.plane, G::CC, G::HR, 1) &&
+              make_map(&c->tm_rti, rt0, c->n_r, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, TI, RC_NT, 1) &&
+              make_map(&c->tm_rth, rt0 + (size_t)RC_NT * y.pitch, c->n_r - 1, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, G::CC, RC_NT, 1);
+    if (!ok) return false;
+    if (cudaFuncSetAttribute(step_kernel_f64_rc<TI, TJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::TOTAL) != cudaSuccess)
+        return false;
+    c->ti = TI; c->tj = TJ; c->smem = G::TOTAL; c->threads = 256;
+    c->grid = dim3((c->n_r + TI - 1) / TI, (c->n_theta + TJ - 1) / TJ);
+    return true;
+}
+
 static int choose_geometry(teuk_ctx* c) {
     c->use_tma = false;
+    c->use_rc = false;
+    if (c->L == 1 && c->coef_variant == 1) {
+        bool ok = (c->opt_tj == 8) ? setup_rc<32, 8>(c) : setup_rc<32, 16>(c);
+        cudaGetLastError();
+        if (!ok) return TEUK_ECUDA;       // the recompute variant exists only as a TMA kernel
+        c->use_rc = true;
+        return TEUK_OK;
+    }
     if (c->L == 1 && c->opt_tma && (c->opt_ti == 0 || c->opt_ti == 32) && (c->opt_tj == 0 || c->opt_tj == 8 || c->opt_tj == 16)) {
         bool ok = (c->opt_tj == 8) ? setup_tma<32, 8>(c) : setup_tma<32, 16>(c);
         cudaGetLastError();
@@ -402,7 +459,11 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
     P.obs_cap = c->obs_cap;
     P.step_off = step_off;
     P.oi = c->oi; P.oj = c->oj;
-    if (c->use_tma) {
+    if (c->use_rc) {
+        RcParams Q{c->dptr(c->lay.rc_th)};
+        if (c->tj == 8) step_kernel_f64_rc<32, 8><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);
+        else step_kernel_f64_rc<32, 16><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);
+    } else if (c->use_tma) {
         if (c->tj == 8) step_kernel_f64_tma<32, 8><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ch, c->tm_ci, P);
         else step_kernel_f64_tma<32, 16><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ch, c->tm_ci, P);
     } else {
@@ -588,6 +649,32 @@ extern "C" int teuk_get_tables(teuk_ctx* c, int half, double* host_out) {
     cudaFree(tmp);
     if (rc != TEUK_OK) return rc;
     for (int pl = 0; pl < 8 * c->L; ++pl)
+        for (int j = 0; j < c->n_theta; ++j)
+            for (int i = 0; i < rows; ++i)
+                host_out[((size_t)pl * c->n_theta + j) * rows + i] = h[(size_t)pl * c->lay.plane + (size_t)j * c->lay.pitch + i];
+    return TEUK_OK;
+}
+
+extern "C" int teuk_get_folded(teuk_ctx* c, int half, int coef_variant, double* host_out) {
+    if (!c || !host_out || c->L != 1 || coef_variant < 0 || coef_variant > 1) return TEUK_EINVAL;
+    int rows = half ? c->n_r - 1 : c->n_r;
+    size_t n = (size_t)8 * c->lay.plane;
+    std::vector<double> h(n);
+    const double* src = c->dptr(half ? c->lay.coef_h : c->lay.coef_i);
+    double* tmp = nullptr;
+    if (coef_variant == 1) {
+        if (cudaMalloc(&tmp, n * 8) != cudaSuccess) return TEUK_ENOMEM;
+        rc_tables_kernel<<<dim3((rows + 127) / 128, c->n_theta), 128, 0, c->stream>>>(
+            c->dptr(c->lay.rc_isig) + (size_t)(half ? 1 : 0) * c->lay.plane,
+            c->dptr(c->lay.rc_rt) + (size_t)(half ? 1 : 0) * RC_NT * c->lay.pitch, c->dptr(c->lay.rc_th), rows, c->n_theta,
+            c->lay.pitch, c->lay.plane, tmp);
+        src = tmp;
+    }
+    cudaError_t e = cudaMemcpyAsync(h.data(), src, n * 8, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (tmp) cudaFree(tmp);
+    if (e != cudaSuccess) return TEUK_ECUDA;
+    for (int pl = 0; pl < 8; ++pl)
         for (int j = 0; j < c->n_theta; ++j)
             for (int i = 0; i < rows; ++i)
                 host_out[((size_t)pl * c->n_theta + j) * rows + i] = h[(size_t)pl * c->lay.plane + (size_t)j * c->lay.pitch + i];

@@ -41,6 +41,7 @@ SIGNATURES = {
     "teuk_destroy": (None, [_h]),
     "teuk_strerror": (C.c_char_p, [C.c_int]),
     "teuk_get_tables": (C.c_int, [_h, C.c_int, _dp]),
+    "teuk_get_folded": (C.c_int, [_h, C.c_int, C.c_int, _dp]),
     "teuk_get_radial": (C.c_int, [_h, _dp, _dp]),
     "teuk_test_mp_op": (C.c_int, [C.c_int, C.c_int, _dp, _dp, _dp, C.c_long, C.c_int]),
     "teuk_test_mp_fn": (C.c_int, [C.c_int, _dp, _dp]),
@@ -183,6 +184,12 @@ class Teuk:
         rows = self.n_r - 1 if half else self.n_r
         out = np.zeros((8, self.L, self.n_theta, rows))
         _chk(lib.teuk_get_tables(self.h, int(half), _np(out)), "teuk_get_tables")
+        return out
+
+    def folded(self, half: bool, coef_variant: int) -> np.ndarray:
+        rows = self.n_r - 1 if half else self.n_r
+        out = np.zeros((8, self.n_theta, rows))
+        _chk(lib.teuk_get_folded(self.h, int(half), coef_variant, _np(out)), "teuk_get_folded")
         return out
 
     def radial(self):

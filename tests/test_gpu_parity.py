@@ -163,6 +163,48 @@ def test_tma_kernel_matches_generic_kernel_fp64(teuk, n_r, n_t):
     assert np.array_equal(outs["tma16"][0], outs["tma8"][0])
 
 
+# ------------------------------------------------------------------------------- semi-recompute coefficient supply (H1b)
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_recomputed_coefficients_match_stored_planes(teuk, cfg):
+    """coef_variant 1 rebuilds the folded coefficients from one 1/Sigma plane + 1-D tables; they must agree with
+    the stored planes (rounded from quad-double) to a few ulps of the largest coefficient at the point"""
+    w = inputs.config(cfg).scaled(n_r=257)
+    g = teuk.Teuk.from_workload(w)
+    for half in (False, True):
+        a, b = g.folded(half, 0), g.folded(half, 1)
+        scale = np.abs(a).max(axis=0, keepdims=True)
+        rel = np.abs(a - b) / np.maximum(np.abs(a), scale / 16)
+        assert rel.max() <= 16 * 2.0 ** -52, (half, float(rel.max()), np.unravel_index(rel.argmax(), rel.shape))
+
+
+@pytest.mark.parametrize("n_r,n_t,base", [(203, 13, 2), (512, 16, 1), (1000, 70, 2), (40, 3, 2)])
+def test_recompute_kernel_parity_fp64(teuk, n_r, n_t, base):
+    w = inputs.config(base).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0)
+    w = w.scaled(dt_override=inputs.stable_dt(w))
+    u0 = inputs.random_state(n_r, n_t, 1, seed=33)
+    o = run_oracle(w, u0, 200, observer=(10.3, 1.1))
+    ref, sref = o.read(), o.observe(200)
+    for opts in ({"coef_variant": 1}, {"coef_variant": 1, "tile_j": 8}):
+        g = run_gpu(teuk, w, u0, 200, options=opts, observer=(10.3, 1.1))
+        err = oracle.rel_linf(g.read(), ref)
+        serr = series_err(g.observe(200), sref)
+        print(n_r, n_t, opts, err, serr)
+        assert max(err.values()) <= TOL[1] and max(serr.values()) <= TOL[1]
+
+
+def test_recompute_kernel_config2_prefix(teuk):
+    w = inputs.config(2)
+    u0 = inputs.initial_state(w)
+    steps = 1000
+    g = run_gpu(teuk, w, u0, steps, options={"coef_variant": 1})
+    o = run_oracle(w, u0, steps)
+    err = oracle.rel_linf(g.read(), o.read())
+    print("cfg2 1000-step prefix, recompute supply:", err)
+    assert max(err.values()) <= TOL[1]
+    with pytest.raises(teuk.TeukError):
+        teuk.Teuk.from_workload(inputs.config(3).scaled(n_r=64)).set_option("coef_variant", 1)   # fp64 only
+
+
 # ------------------------------------------------------------------------------- full-size configs (bench launch geometry)
 @pytest.mark.parametrize("cfg,steps_gpu,k", [(2, 300, 12), (3, 120, 8), (4, 100, 6)])
 def test_full_size_configs_windowed(teuk, cfg, steps_gpu, k):
@@ -224,16 +266,20 @@ def test_config2_prefix_full_grid_fp64(teuk):
                     reason="7 minutes of host time for the full-grid oracle; set TEUK_FULL_LENGTH=1 "
                            "(measured on B200: Phi 2.1e-14, Pi 8.9e-13, observer 2.8e-14; DESIGN.md section 5)")
 def test_config2_full_length_fp64(teuk):
-    """BASELINE.json config 2 at full size AND full length (20000 steps) against the full-grid oracle."""
+    """BASELINE.json config 2 at full size AND full length (20000 steps) against the full-grid oracle,
+    for both coefficient supplies (stored planes; semi-recompute)."""
     w = inputs.config(2)
     u0 = inputs.initial_state(w)
-    g = run_gpu(teuk, w, u0, w.steps, observer=w.observer)
     o = run_oracle(w, u0, w.steps, observer=w.observer)
-    err = oracle.rel_linf(g.read(), o.read())
-    serr = series_err(g.observe(w.steps), o.observe(w.steps))
-    print("cfg2 full length: state", err, "observer", serr)
-    assert max(err.values()) <= TOL[1]
-    assert max(serr.values()) <= TOL[1]
+    ref, sref = o.read(), o.observe(w.steps)
+    res = {}
+    for cv in (0, 1):
+        g = run_gpu(teuk, w, u0, w.steps, observer=w.observer, options={"coef_variant": cv})
+        res[cv] = (oracle.rel_linf(g.read(), ref), series_err(g.observe(w.steps), sref))
+        print("cfg2 full length, coef_variant", cv, ": state", res[cv][0], "observer", res[cv][1])
+    for cv in (0, 1):
+        assert max(res[cv][0].values()) <= TOL[1], cv
+        assert max(res[cv][1].values()) <= TOL[1], cv
 
 
 # ------------------------------------------------------------------------------- invariants and edge cases
