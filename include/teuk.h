@@ -42,7 +42,9 @@ int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double r
 /* Options, only before teuk_set_initial (else TEUK_ESTATE): "graph_steps" (even, >= 2; steps per
  * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic), "use_tma" (fp64: 1 = TMA
  * kernel, default; 0 = generic kernel), "variant" (dd/qd launch shape 0..2), "coef_variant" (0 = precomputed
- * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only). */
+ * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only),
+ * "theta_order" (2 = second-order centred theta differences, default; 10 = the 10th-order
+ * 11-point operator of PAPER.md:126, needs n_theta >= 5). */
 int teuk_set_option(teuk_ctx *, const char *key, double value);
 
 /* Observer at a fixed location: bilinear interpolation in (r*, theta) from the four

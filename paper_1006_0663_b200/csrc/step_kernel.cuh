@@ -70,6 +70,17 @@ template <int L> struct GlobalCoef {       // coefficient q straight from the gl
     __device__ __forceinline__ Real<L> get(int q) const { return Ld<L>::g(p + (long)q * L * stride, stride, idx); }
 };
 
+// Weights of the wide (10th-order) theta stencils as quad-double limbs; narrowed to L in the kernel.
+struct ThetaWeights {
+    double wd[6][4];     // second derivative, k = 0..5 (units 1/dtheta^2)
+    double wc[5][4];     // first derivative, k = 1..5 (units 1/dtheta)
+};
+
+template <int L, class Tile, class Coef>
+__device__ __forceinline__ void substep_core(const Real<L> sg[4], const Real<L> dl[4], const Real<L> lam[2], const Coef& cf,
+                                             double tq, bool half, const Real<L> base_in[4], Real<L> out[4]);
+
+// stencil half-width 1: Lam = ((sig+ + sig-) - 2 sig) + cj (sig+ - sig-)
 template <int L, class Tile, class Coef>
 __device__ __forceinline__ void substep(const Tile& t, int row, int rm, int rp, double sm, double sp, int clo, int chi,
                                         const Coef& cf, const Real<L>& cjv,
@@ -91,6 +102,53 @@ __device__ __forceinline__ void substep(const Tile& t, int row, int rm, int rp, 
         Real<L> first = mul(cjv, sub(up, dn));
         lam[c] = add(second, first);
     }
+    substep_core<L, Tile, Coef>(sg, dl, lam, cf, tq, half, base_in, out);
+}
+
+// stencil half-width 5 (10th order):  Lam = d0 sig + sum_k d_k (sig_{+k} + sig_{-k}) + 2 cj sum_k c_k (sig_{+k} - sig_{-k}),
+// ghost rows mirrored about the axis with sign sigma (f_{-k} = sigma f_{k-1}, f_{N-1+k} = sigma f_{N-k}).
+// The tile must hold every theta row (column kernel below).
+template <int L, class Tile, class Coef>
+__device__ __forceinline__ void substep_wide(const Tile& t, int row, int nt, double sigma, int clo, int chi, const Coef& cf,
+                                             const Real<L>& cjv, const ThetaWeights& W, double tq, bool half,
+                                             const Real<L> base_in[4], Real<L> out[4]) {
+    Real<L> sg[4], dl[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        Real<L> lo = t.get(c, row, clo), hi = t.get(c, row, chi);
+        sg[c] = add(hi, lo);
+        dl[c] = sub(hi, lo);
+    }
+    Real<L> lam[2];
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        Real<L> w0;
+#pragma unroll
+        for (int l = 0; l < L; ++l) w0.x[l] = W.wd[0][l];
+        Real<L> s2 = mul(w0, sg[c]);
+        Real<L> s1 = from_double<L>(0.0);
+#pragma unroll 1
+        for (int k = 1; k <= 5; ++k) {
+            int ru = row + k, rd = row - k;
+            double su = 1.0, sd = 1.0;
+            if (ru >= nt) { ru = 2 * nt - 1 - ru; su = sigma; }
+            if (rd < 0) { rd = -rd - 1; sd = sigma; }
+            Real<L> up = sgn(add(t.get(c, ru, chi), t.get(c, ru, clo)), su);
+            Real<L> dn = sgn(add(t.get(c, rd, chi), t.get(c, rd, clo)), sd);
+            Real<L> wd, wc;
+#pragma unroll
+            for (int l = 0; l < L; ++l) { wd.x[l] = W.wd[k][l]; wc.x[l] = W.wc[k - 1][l]; }
+            s2 = add(s2, mul(wd, add(up, dn)));
+            s1 = add(s1, mul(wc, sub(up, dn)));
+        }
+        lam[c] = add(s2, mul(cjv, scale2(s1, 2.0)));
+    }
+    substep_core<L, Tile, Coef>(sg, dl, lam, cf, tq, half, base_in, out);
+}
+
+template <int L, class Tile, class Coef>
+__device__ __forceinline__ void substep_core(const Real<L> sg[4], const Real<L> dl[4], const Real<L> lam[2], const Coef& cf,
+                                             double tq, bool half, const Real<L> base_in[4], Real<L> out[4]) {
     Real<L> c0 = cf.get(0);
     Real<L> c1 = cf.get(1);
     Real<L> c2 = cf.get(2);
@@ -265,6 +323,85 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel(StepParams P) {
         }
         if (PF) cc = cn;
         idx = nidx; tc = ntc; tr = ntr; gi = ngi; gj = ngj; v = nv; interior = ninterior;
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
+// Column kernel for the 10th-order theta operator (NEXT-1): a block owns TI radial columns and ALL
+// N_theta rows, so the +-5-row reach of each sub-step needs no theta halo (ghost rows are mirrored reads) and the
+// only redundant work is the one extra half-step column per block, (TI+1)/TI.  Same fusion as step_kernel.
+template <int L, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) step_kernel_col(StepParams P, ThetaWeights W) {
+    extern __shared__ double smem[];
+    const int TI = P.ti, nt = P.n_theta, nr = P.n_r;
+    const int UC = TI + 2, HC = TI + 1;
+    double* us = smem;                       // [4L][nt][UC]
+    double* hs = smem + 4 * L * nt * UC;     // [4L][nt][HC]
+    const int i0 = blockIdx.x * TI, iu0 = i0 - 1;
+    const int tid = threadIdx.x, nth = MAXT;
+
+    for (int k = tid; k < 4 * L * nt * UC; k += nth) {
+        int c = k % UC, rest = k / UC;
+        int r = rest % nt, pl = rest / nt;
+        int ui = iu0 + c;
+        double val = 0.0;
+        if (ui >= 0 && ui < nr) val = __ldg(P.u_in + pl * P.plane + (long)r * P.pitch + ui);
+        us[k] = val;
+    }
+    __syncthreads();
+
+    SmemTile<L> ut{us, nt, UC, 0};
+    for (int idx = tid; idx < nt * HC; idx += nth) {
+        int tr = idx / HC, tc = idx - tr * HC;
+        int ih = iu0 + tc;
+        if (ih < 0 || ih > nr - 2) continue;
+        RegCoef<L> cc;
+        load_coef(cc, P.coef_h, P.plane, (long)tr * P.pitch + ih);
+        Real<L> cjv = Ld<L>::g(P.cj, nt, tr);
+        Real<L> out[4];
+        substep_wide<L>(ut, tr, nt, P.sigma, tc, tc + 1, cc, cjv, W, P.tq_half, true, out, out);
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int l = 0; l < L; ++l) hs[(c * L + l) * nt * HC + tr * HC + tc] = out[c].x[l];
+    }
+    __syncthreads();
+
+    SmemTile<L> ht{hs, nt, HC, 0};
+    for (int idx = tid; idx < nt * TI; idx += nth) {
+        int tr = idx / TI, tc = idx - tr * TI;
+        int i = i0 + tc, j = tr;
+        if (i >= nr) continue;
+        Real<L> out[4];
+        if (i == 0 || i == nr - 1) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) out[c] = from_double<L>(0.0);
+        } else {
+            RegCoef<L> cc;
+            load_coef(cc, P.coef_i, P.plane, (long)j * P.pitch + i);
+            Real<L> base[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) base[c] = ut.get(c, j, tc + 1);
+            Real<L> cjv = Ld<L>::g(P.cj, nt, j);
+            substep_wide<L>(ht, j, nt, P.sigma, tc, tc + 1, cc, cjv, W, P.tq_full, false, base, out);
+        }
+        long g = (long)j * P.pitch + i;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) Ld<L>::st(P.u_out + (long)c * L * P.plane, P.plane, g, out[c]);
+        if (P.obs_raw != nullptr) {
+            int di = i - P.oi, dj = j - P.oj;
+            if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
+                long k = *P.step_base + P.step_off;
+                if (k < P.obs_cap) {
+                    double* o = P.obs_raw + ((k * 4 + (dj * 2 + di)) * 4) * L;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+#pragma unroll
+                        for (int l = 0; l < L; ++l) o[c * L + l] = out[c].x[l];
+                }
+            }
+        }
     }
 }
 

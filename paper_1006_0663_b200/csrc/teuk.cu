@@ -75,7 +75,8 @@ struct teuk_ctx {
     cudaStream_t stream;
     SetupConsts C;
     // options
-    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0;
+    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0, theta_order = 2;
+    ThetaWeights tw;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
     bool use_tma = false, use_rc = false;
     CUtensorMap tm_state[2], tm_ch, tm_ci, tm_ish, tm_isi, tm_rth, tm_rti;
@@ -295,6 +296,9 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     } else if (!strcmp(key, "tile_j")) {
         if (v < 0 || v > 256) return TEUK_EINVAL;
         c->opt_tj = v;
+    } else if (!strcmp(key, "theta_order")) {
+        if ((v != 2 && v != 10) || c->n_theta < v / 2) return TEUK_EINVAL;
+        c->theta_order = v;
     } else if (!strcmp(key, "coef_variant")) {
         if (v < 0 || v > 1 || (v == 1 && c->L != 1)) return TEUK_EINVAL;
         c->coef_variant = v;
@@ -408,9 +412,52 @@ template <int TI, int TJ> static bool setup_rc(teuk_ctx* c) {
     return true;
 }
 
+static const void* col_fn(const teuk_ctx* c, int* threads) {
+    *threads = 256;
+    if (c->L == 1) return (const void*)step_kernel_col<1, 256, 2>;
+    if (c->L == 2) return (const void*)step_kernel_col<2, 256, 2>;
+    *threads = 128;
+    return (const void*)step_kernel_col<4, 128, 3>;
+}
+
+// centred 11-point weights from the textbook closed form c_k = (-1)^(k+1) (N!)^2 / (k (N-k)! (N+k)!), d_k = 2 c_k / k
+static void fill_theta_weights(ThetaWeights& w) {
+    const int N = 5;
+    double fact[11] = {1, 1, 2, 6, 24, 120, 720, 5040, 40320, 362880, 3628800};
+    R4 d0 = from_double<4>(0.0);
+    for (int k = 1; k <= N; ++k) {
+        R4 num = from_double<4>(((k & 1) ? 1.0 : -1.0) * fact[N] * fact[N]);
+        R4 den = from_double<4>((double)k * fact[N - k] * fact[N + k]);
+        R4 ck = div(num, den);
+        R4 dk = div(scale2(ck, 2.0), from_double<4>((double)k));
+        d0 = sub(d0, scale2(dk, 2.0));
+        for (int l = 0; l < 4; ++l) { w.wc[k - 1][l] = ck.x[l]; w.wd[k][l] = dk.x[l]; }
+    }
+    for (int l = 0; l < 4; ++l) w.wd[0][l] = d0.x[l];
+}
+
 static int choose_geometry(teuk_ctx* c) {
     c->use_tma = false;
     c->use_rc = false;
+    if (c->theta_order == 10) {
+        if (c->coef_variant != 0) return TEUK_EINVAL;
+        fill_theta_weights(c->tw);
+        int ti = c->opt_ti;
+        if (ti == 0) {
+            // largest tile that keeps ~3 blocks/SM worth of shared memory (72 KB per block)
+            long per_col = (long)4 * c->L * 8 * c->n_theta;       // bytes per tile column, u or h
+            ti = (int)((72 * 1024 / per_col - 3) / 2);
+            if (ti > 32) ti = 32;
+            if (ti < 2) ti = 2;
+        }
+        if (ti > c->n_r) ti = c->n_r;
+        size_t sm = (size_t)4 * c->L * 8 * c->n_theta * (2 * ti + 3);
+        if (sm > 227 * 1024) return TEUK_EINVAL;
+        c->ti = ti; c->tj = c->n_theta; c->smem = sm;
+        c->grid = dim3((c->n_r + ti - 1) / ti, 1);
+        const void* fn = col_fn(c, &c->threads);
+        return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+    }
     if (c->L == 1 && c->coef_variant == 1) {
         bool ok = (c->opt_tj == 8) ? setup_rc<32, 8>(c) : setup_rc<32, 16>(c);
         cudaGetLastError();
@@ -459,7 +506,12 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
     P.obs_cap = c->obs_cap;
     P.step_off = step_off;
     P.oi = c->oi; P.oj = c->oj;
-    if (c->use_rc) {
+    if (c->theta_order == 10) {
+        void* args[] = {&P, &c->tw};
+        int threads = 256;
+        const void* fn = col_fn(c, &threads);
+        if (cudaLaunchKernel(fn, c->grid, dim3(threads), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
+    } else if (c->use_rc) {
         RcParams Q{c->dptr(c->lay.rc_th)};
         if (c->tj == 8) step_kernel_f64_rc<32, 8><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);
         else step_kernel_f64_rc<32, 16><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);

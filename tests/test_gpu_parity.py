@@ -205,6 +205,72 @@ def test_recompute_kernel_config2_prefix(teuk):
         teuk.Teuk.from_workload(inputs.config(3).scaled(n_r=64)).set_option("coef_variant", 1)   # fp64 only
 
 
+# ------------------------------------------------------------------------------- NEXT-1: 10th-order theta operator
+@pytest.mark.parametrize("L,n_r,n_t,steps,base", [(1, 203, 13, 200, 2), (2, 203, 13, 100, 2), (4, 131, 11, 40, 2),
+                                                  (1, 300, 64, 100, 2), (2, 150, 32, 40, 4), (4, 90, 32, 20, 4),
+                                                  (1, 64, 5, 50, 2)])
+def test_theta10_parity_all_precisions(teuk, L, n_r, n_t, steps, base):
+    """10th-order angular operator, rest of the scheme unchanged; column kernel vs oracle"""
+    w = inputs.config(base).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0, precision=L)
+    w = w.scaled(dt_override=0.5 * inputs.stable_dt(w))       # the wide stencil's largest eigenvalue is ~1.7x larger
+    u0 = inputs.random_state(n_r, n_t, L, seed=200 + L)
+    obs = (10.3, 1.1)
+    g = run_gpu(teuk, w, u0, steps, observer=obs, options={"theta_order": 10})
+    o = oracle.Oracle.from_workload(w, theta_order=10)
+    o.set_observer(obs[0], obs[1], steps)
+    o.set_initial(u0)
+    o.step(steps)
+    err = oracle.rel_linf(g.read(), o.read())
+    serr = series_err(g.observe(steps), o.observe(steps))
+    print("theta10", L, n_r, n_t, err, serr)
+    assert max(err.values()) <= TOL[L] and max(serr.values()) <= TOL[L]
+    # the option is live: the 2nd-order kernel gives a different answer
+    g2 = run_gpu(teuk, w, u0, steps)
+    assert not np.array_equal(g2.read(), g.read())
+
+
+def test_theta10_invariants_and_tiles(teuk):
+    w = inputs.config(1).scaled(n_r=96, precision=2)
+    u0 = inputs.initial_state(w)
+    u = run_gpu(teuk, w, u0, 40, options={"theta_order": 10}).read()
+    assert np.array_equal(u, u[:, :, ::-1, :])
+    assert not u[..., 0].any() and not u[..., -1].any() and not u[1].any()
+    for ti in (2, 5, 16):
+        v = run_gpu(teuk, w, u0, 40, options={"theta_order": 10, "tile_i": ti}).read()
+        assert np.array_equal(u, v)
+    h = teuk.Teuk.from_workload(w.scaled(n_theta=4))
+    with pytest.raises(teuk.TeukError):
+        h.set_option("theta_order", 10)          # needs n_theta >= 5
+
+
+@pytest.mark.parametrize("cfg,steps_gpu,k", [(2, 100, 8), (3, 60, 6), (4, 60, 4)])
+def test_theta10_full_size_configs_windowed(teuk, cfg, steps_gpu, k):
+    w = inputs.config(cfg)
+    w = w.scaled(dt_override=0.5 * w.dt)
+    L = w.precision
+    u0 = inputs.initial_state(w)
+    g = run_gpu(teuk, w, u0, steps_gpu, options={"theta_order": 10})
+    mid = g.read()
+    assert np.isfinite(mid).all()
+    g.step(k)
+    fin = g.read()
+    i_c = int((inputs.pulse_parameters(w)[0] - w.rstar_min) / w.dr)
+    n_win = 64
+    for i_lo in (0, i_c - n_win // 2, w.n_r - n_win):
+        o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win, theta_order=10)
+        o.set_initial(np.ascontiguousarray(mid[..., i_lo:i_lo + n_win]))
+        o.step(k)
+        ref = o.read()
+        a, b = (0 if i_lo == 0 else k + 1), (n_win if i_lo + n_win == w.n_r else n_win - k - 1)
+        got = np.ascontiguousarray(fin[..., i_lo:i_lo + n_win][..., a:b])
+        want = np.ascontiguousarray(ref[..., a:b])
+        for re, im in ((0, 1), (2, 3)):
+            dre, _ = oracle._limb_diff(got[re], want[re])
+            dim, _ = oracle._limb_diff(got[im], want[im])
+            den = np.hypot(fin[re, 0], fin[im, 0]).max()
+            assert float(np.hypot(dre, dim).max() / den) <= TOL[L], (cfg, i_lo, re)
+
+
 # ------------------------------------------------------------------------------- full-size configs (bench launch geometry)
 @pytest.mark.parametrize("cfg,steps_gpu,k", [(2, 300, 12), (3, 120, 8), (4, 100, 6)])
 def test_full_size_configs_windowed(teuk, cfg, steps_gpu, k):
