@@ -325,6 +325,21 @@ def main():
             per[name] = {"precision_limbs": wx.precision, "n_r": wx.n_r, "n_theta": wx.n_theta, "steps": k_steps,
                          "updates_per_s": wx.n_r * wx.n_theta * k_steps / (msx * 1e-3), "ms_per_step": msx / k_steps,
                          "geometry": gx, "finite": fx}
+        # NEXT-1: the same three workloads with the 10th-order theta operator (column kernel)
+        t10 = {}
+        for name, k_steps in (("cfg2", max(50, args.steps // 10)), ("cfg3", max(50, args.steps // 10)), ("cfg4", max(50, args.steps // 10))):
+            wx = workload(name)
+            wx = wx.scaled(dt_override=0.5 * wx.dt)
+            msx, lx, gx, fx = time_device(torch, teuk, wx, k_steps, 20, list(args.option) + ["theta_order=10"])
+            t10[name] = {"precision_limbs": wx.precision, "steps": k_steps, "updates_per_s": wx.n_r * wx.n_theta * k_steps / (msx * 1e-3),
+                         "ms_per_step": msx / k_steps, "geometry": gx, "finite": fx}
+        line["theta_order_10"] = t10
+        # H1b variant (b): semi-recompute coefficient supply for the primary workload (80 B/update)
+        if L == 1:
+            msr, lr, gr, fr = time_device(torch, teuk, w, args.steps, args.warmup, list(args.option) + ["coef_variant=1"])
+            ach = 80.0 * points / (msr / args.steps * 1e-3) / 1e9
+            line["semi_recompute"] = {"updates_per_s": points * args.steps / (msr * 1e-3), "ms_per_step": msr / args.steps,
+                                      "algorithmic_bytes_per_update": 80.0, "hbm_frac": ach / peak, "geometry": gr, "finite": fr}
         line["per_precision"] = per
         line["fp64_pipe_peak_inst_per_s"] = fp
         line["cpu_baseline"] = cpu_baseline(w)

@@ -109,14 +109,15 @@ __device__ __forceinline__ void substep(const Tile& t, int row, int rm, int rp, 
 // ghost rows mirrored about the axis with sign sigma (f_{-k} = sigma f_{k-1}, f_{N-1+k} = sigma f_{N-k}).
 // The tile must hold every theta row (column kernel below).
 template <int L, class Tile, class Coef>
-__device__ __forceinline__ void substep_wide(const Tile& t, int row, int nt, double sigma, int clo, int chi, const Coef& cf,
-                                             const Real<L>& cjv, const ThetaWeights& W, double tq, bool half,
-                                             const Real<L> base_in[4], Real<L> out[4]) {
+__device__ __forceinline__ void substep_wide(const Tile& t, const Tile& st, int scol, int row, int nt, double sigma, int clo,
+                                             int chi, const Coef& cf, const Real<L>& cjv, const ThetaWeights& W, double tq,
+                                             bool half, const Real<L> base_in[4], Real<L> out[4]) {
+    // st: staged tile of sig_Phi = Phi_hi + Phi_lo (2 components) at every row, column scol <-> this point
     Real<L> sg[4], dl[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
         Real<L> lo = t.get(c, row, clo), hi = t.get(c, row, chi);
-        sg[c] = add(hi, lo);
+        sg[c] = (c < 2) ? st.get(c, row, scol) : add(hi, lo);
         dl[c] = sub(hi, lo);
     }
     Real<L> lam[2];
@@ -133,8 +134,8 @@ __device__ __forceinline__ void substep_wide(const Tile& t, int row, int nt, dou
             double su = 1.0, sd = 1.0;
             if (ru >= nt) { ru = 2 * nt - 1 - ru; su = sigma; }
             if (rd < 0) { rd = -rd - 1; sd = sigma; }
-            Real<L> up = sgn(add(t.get(c, ru, chi), t.get(c, ru, clo)), su);
-            Real<L> dn = sgn(add(t.get(c, rd, chi), t.get(c, rd, clo)), sd);
+            Real<L> up = sgn(st.get(c, ru, scol), su);
+            Real<L> dn = sgn(st.get(c, rd, scol), sd);
             Real<L> wd, wc;
 #pragma unroll
             for (int l = 0; l < L; ++l) { wd.x[l] = W.wd[k][l]; wc.x[l] = W.wc[k - 1][l]; }
@@ -338,6 +339,7 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel_col(StepParams P, Thet
     const int UC = TI + 2, HC = TI + 1;
     double* us = smem;                       // [4L][nt][UC]
     double* hs = smem + 4 * L * nt * UC;     // [4L][nt][HC]
+    double* ss = hs + 4 * L * nt * HC;       // [2L][nt][HC]  staged sig_Phi = Phi_hi + Phi_lo (each sum formed once, used 11x)
     const int i0 = blockIdx.x * TI, iu0 = i0 - 1;
     const int tid = threadIdx.x, nth = MAXT;
 
@@ -352,6 +354,15 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel_col(StepParams P, Thet
     __syncthreads();
 
     SmemTile<L> ut{us, nt, UC, 0};
+    for (int idx = tid; idx < 2 * nt * HC; idx += nth) {
+        int tc = idx % HC, rest = idx / HC;
+        int tr = rest % nt, c = rest / nt;
+        Real<L> sgm = add(ut.get(c, tr, tc + 1), ut.get(c, tr, tc));
+#pragma unroll
+        for (int l = 0; l < L; ++l) ss[(c * L + l) * nt * HC + tr * HC + tc] = sgm.x[l];
+    }
+    __syncthreads();
+    SmemTile<L> st1{ss, nt, HC, 0};
     for (int idx = tid; idx < nt * HC; idx += nth) {
         int tr = idx / HC, tc = idx - tr * HC;
         int ih = iu0 + tc;
@@ -360,7 +371,7 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel_col(StepParams P, Thet
         load_coef(cc, P.coef_h, P.plane, (long)tr * P.pitch + ih);
         Real<L> cjv = Ld<L>::g(P.cj, nt, tr);
         Real<L> out[4];
-        substep_wide<L>(ut, tr, nt, P.sigma, tc, tc + 1, cc, cjv, W, P.tq_half, true, out, out);
+        substep_wide<L>(ut, st1, tc, tr, nt, P.sigma, tc, tc + 1, cc, cjv, W, P.tq_half, true, out, out);
 #pragma unroll
         for (int c = 0; c < 4; ++c)
 #pragma unroll
@@ -369,6 +380,15 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel_col(StepParams P, Thet
     __syncthreads();
 
     SmemTile<L> ht{hs, nt, HC, 0};
+    for (int idx = tid; idx < 2 * nt * TI; idx += nth) {      // sig of the half-step field, [2L][nt][TI]
+        int tc = idx % TI, rest = idx / TI;
+        int tr = rest % nt, c = rest / nt;
+        Real<L> sgm = add(ht.get(c, tr, tc + 1), ht.get(c, tr, tc));
+#pragma unroll
+        for (int l = 0; l < L; ++l) ss[(c * L + l) * nt * TI + tr * TI + tc] = sgm.x[l];
+    }
+    __syncthreads();
+    SmemTile<L> st2{ss, nt, TI, 0};
     for (int idx = tid; idx < nt * TI; idx += nth) {
         int tr = idx / TI, tc = idx - tr * TI;
         int i = i0 + tc, j = tr;
@@ -384,7 +404,7 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel_col(StepParams P, Thet
 #pragma unroll
             for (int c = 0; c < 4; ++c) base[c] = ut.get(c, j, tc + 1);
             Real<L> cjv = Ld<L>::g(P.cj, nt, j);
-            substep_wide<L>(ht, j, nt, P.sigma, tc, tc + 1, cc, cjv, W, P.tq_full, false, base, out);
+            substep_wide<L>(ht, st2, tc, j, nt, P.sigma, tc, tc + 1, cc, cjv, W, P.tq_full, false, base, out);
         }
         long g = (long)j * P.pitch + i;
 #pragma unroll

@@ -444,14 +444,15 @@ static int choose_geometry(teuk_ctx* c) {
         fill_theta_weights(c->tw);
         int ti = c->opt_ti;
         if (ti == 0) {
-            // largest tile that keeps ~3 blocks/SM worth of shared memory (72 KB per block)
-            long per_col = (long)4 * c->L * 8 * c->n_theta;       // bytes per tile column, u or h
-            ti = (int)((72 * 1024 / per_col - 3) / 2);
+            // largest tile within the shared-memory budget: 3 blocks/SM for qd (72 KB each), 2 blocks/SM otherwise (100 KB)
+            long per_col = (long)4 * c->L * 8 * c->n_theta;       // bytes per tile column of u or h (sig tile: half of that)
+            ti = (int)(((c->L == 4 ? 72 : 100) * 1024 / per_col - 3.5) / 2.5);
             if (ti > 32) ti = 32;
+            if (c->L == 1 && ti >= 8) ti = (ti >= 16) ? 16 : 8;      // fp64: whole 64/128-byte rows per tile (measured best)
             if (ti < 2) ti = 2;
         }
         if (ti > c->n_r) ti = c->n_r;
-        size_t sm = (size_t)4 * c->L * 8 * c->n_theta * (2 * ti + 3);
+        size_t sm = (size_t)4 * c->L * 8 * c->n_theta * (2 * ti + 3) + (size_t)2 * c->L * 8 * c->n_theta * (ti + 1);
         if (sm > 227 * 1024) return TEUK_EINVAL;
         c->ti = ti; c->tj = c->n_theta; c->smem = sm;
         c->grid = dim3((c->n_r + ti - 1) / ti, 1);
