@@ -108,8 +108,8 @@ __device__ __forceinline__ void substep(const Tile& t, int row, int rm, int rp, 
 // stencil half-width 5 (10th order):  Lam = d0 sig + sum_k d_k (sig_{+k} + sig_{-k}) + 2 cj sum_k c_k (sig_{+k} - sig_{-k}),
 // ghost rows mirrored about the axis with sign sigma (f_{-k} = sigma f_{k-1}, f_{N-1+k} = sigma f_{N-k}).
 // The tile must hold every theta row (column kernel below).
-template <int L, class Tile, class Coef>
-__device__ __forceinline__ void substep_wide(const Tile& t, const Tile& st, int scol, int row, int nt, double sigma, int clo,
+template <int L, class Tile, class STile, class Coef>
+__device__ __forceinline__ void substep_wide(const Tile& t, const STile& st, int scol, int row, int nt, double sigma, int clo,
                                              int chi, const Coef& cf, const Real<L>& cjv, const ThetaWeights& W, double tq,
                                              bool half, const Real<L> base_in[4], Real<L> out[4]) {
     // st: staged tile of sig_Phi = Phi_hi + Phi_lo (2 components) at every row, column scol <-> this point
@@ -128,19 +128,34 @@ __device__ __forceinline__ void substep_wide(const Tile& t, const Tile& st, int 
         for (int l = 0; l < L; ++l) w0.x[l] = W.wd[0][l];
         Real<L> s2 = mul(w0, sg[c]);
         Real<L> s1 = from_double<L>(0.0);
-#pragma unroll 1
-        for (int k = 1; k <= 5; ++k) {
-            int ru = row + k, rd = row - k;
-            double su = 1.0, sd = 1.0;
-            if (ru >= nt) { ru = 2 * nt - 1 - ru; su = sigma; }
-            if (rd < 0) { rd = -rd - 1; sd = sigma; }
-            Real<L> up = sgn(st.get(c, ru, scol), su);
-            Real<L> dn = sgn(st.get(c, rd, scol), sd);
-            Real<L> wd, wc;
+        if (L == 1 && row >= 5 && row + 5 < nt) {
+            // fp64 (instruction-bound): rows away from the axis need no mirroring -> straight-line unrolled code;
+            // dd/qd (FP64-pipe bound) keep the single compact loop (the extra code path cost them registers)
 #pragma unroll
-            for (int l = 0; l < L; ++l) { wd.x[l] = W.wd[k][l]; wc.x[l] = W.wc[k - 1][l]; }
-            s2 = add(s2, mul(wd, add(up, dn)));
-            s1 = add(s1, mul(wc, sub(up, dn)));
+            for (int k = 1; k <= 5; ++k) {
+                Real<L> up = st.get(c, row + k, scol);
+                Real<L> dn = st.get(c, row - k, scol);
+                Real<L> wd, wc;
+#pragma unroll
+                for (int l = 0; l < L; ++l) { wd.x[l] = W.wd[k][l]; wc.x[l] = W.wc[k - 1][l]; }
+                s2 = add(s2, mul(wd, add(up, dn)));
+                s1 = add(s1, mul(wc, sub(up, dn)));
+            }
+        } else {
+#pragma unroll 1
+            for (int k = 1; k <= 5; ++k) {
+                int ru = row + k, rd = row - k;
+                double su = 1.0, sd = 1.0;
+                if (ru >= nt) { ru = 2 * nt - 1 - ru; su = sigma; }
+                if (rd < 0) { rd = -rd - 1; sd = sigma; }
+                Real<L> up = sgn(st.get(c, ru, scol), su);
+                Real<L> dn = sgn(st.get(c, rd, scol), sd);
+                Real<L> wd, wc;
+#pragma unroll
+                for (int l = 0; l < L; ++l) { wd.x[l] = W.wd[k][l]; wc.x[l] = W.wc[k - 1][l]; }
+                s2 = add(s2, mul(wd, add(up, dn)));
+                s1 = add(s1, mul(wc, sub(up, dn)));
+            }
         }
         lam[c] = add(s2, mul(cjv, scale2(s1, 2.0)));
     }

@@ -332,6 +332,136 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// fp64 column kernel for the 10th-order theta operator (NEXT-1) with TMA staging and the semi-recompute coefficient
+// supply: a block owns TI columns x all N_theta (<= 256) rows.  Five TMA loads per block (u tile, two 1/Sigma tiles,
+// two r-table slabs), sig_Phi staged once in shared memory, compile-time column counts.
+template <int COLS> struct RTile {              // run-time row count, compile-time column count
+    const double* p;
+    int rows;
+    __device__ __forceinline__ R1 get(int c, int row, int col) const {
+        R1 r;
+        r.x[0] = p[(c * rows + row) * COLS + col];
+        return r;
+    }
+};
+
+template <int TI> struct ColGeom {
+    static constexpr int UC = TI + 4, HC = TI + 1, CC = TI + 2, NT = 16;
+    static size_t a128(size_t v) { return (v + 127) / 128 * 128; }
+    static size_t total(int nt) {
+        return a128((size_t)4 * nt * UC * 8) + a128((size_t)nt * CC * 8) + a128((size_t)nt * TI * 8) + a128((size_t)NT * CC * 8) +
+               a128((size_t)NT * TI * 8) + a128((size_t)4 * nt * HC * 8) + a128((size_t)2 * nt * HC * 8) + 128;
+    }
+};
+
+template <int TI>
+__global__ void __launch_bounds__(256) step_kernel_f64_col_tma(const __grid_constant__ CUtensorMap tm_u,
+                                                              const __grid_constant__ CUtensorMap tm_ish,
+                                                              const __grid_constant__ CUtensorMap tm_isi,
+                                                              const __grid_constant__ CUtensorMap tm_rth,
+                                                              const __grid_constant__ CUtensorMap tm_rti, StepParams P,
+                                                              RcParams Q, ThetaWeights W) {
+    using G = ColGeom<TI>;
+    constexpr int UC = G::UC, HC = G::HC, CC = G::CC, NT = G::NT;
+    extern __shared__ __align__(128) unsigned char raw[];
+    __shared__ __align__(8) uint64_t bar[2];
+    const int nt = P.n_theta, nr = P.n_r;
+    auto a128 = [](size_t v) { return (v + 127) / 128 * 128; };
+    unsigned char* base = (unsigned char*)(((uintptr_t)raw + 127) & ~(uintptr_t)127);
+    double* us = (double*)base;                      base += a128((size_t)4 * nt * UC * 8);
+    double* ish = (double*)base;                     base += a128((size_t)nt * CC * 8);
+    double* isi = (double*)base;                     base += a128((size_t)nt * TI * 8);
+    double* rth = (double*)base;                     base += a128((size_t)NT * CC * 8);
+    double* rti = (double*)base;                     base += a128((size_t)NT * TI * 8);
+    double* hs = (double*)base;                      base += a128((size_t)4 * nt * HC * 8);
+    double* ss = (double*)base;
+    const int i0 = blockIdx.x * TI;
+    const int tid = threadIdx.x;
+
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&bar[0], (4 * nt * UC + nt * CC + NT * CC) * 8);
+        tma_load_3d(us, &tm_u, i0 - 2, 0, 0, &bar[0]);
+        tma_load_3d(ish, &tm_ish, i0 - 2, 0, 0, &bar[0]);
+        tma_load_3d(rth, &tm_rth, i0 - 2, 0, 0, &bar[0]);
+        mbar_expect_tx(&bar[1], (nt * TI + NT * TI) * 8);
+        tma_load_3d(isi, &tm_isi, i0, 0, 0, &bar[1]);
+        tma_load_3d(rti, &tm_rti, i0, 0, 0, &bar[1]);
+    }
+    mbar_wait(&bar[0], 0);
+
+    RTile<UC> ut{us, nt};
+    // sig_Phi = Phi(i+1) + Phi(i) at the TI+1 half points (u tile column of half point tc: tc+1 and tc+2)
+    for (int idx = tid; idx < 2 * nt * HC; idx += 256) {
+        int tc = idx % HC, rest = idx / HC;
+        ss[rest * HC + tc] = us[rest * UC + tc + 2] + us[rest * UC + tc + 1];
+    }
+    __syncthreads();
+    RTile<HC> st1{ss, nt};
+    for (int idx = tid; idx < nt * HC; idx += 256) {
+        int tr = idx / HC, tc = idx - tr * HC;
+        int ih = i0 - 1 + tc;
+        if (ih < 0 || ih > nr - 2) continue;
+        R1 cjv;
+        cjv.x[0] = __ldg(P.cj + tr);
+        RcCoef cf;
+        rc_eval(cf, ish[tr * CC + tc + 1], rth + tc + 1, CC, __ldg(Q.th + tr), __ldg(Q.th + nt + tr), __ldg(Q.th + 2 * nt + tr));
+        R1 out[4];
+        substep_wide<1>(ut, st1, tc, tr, nt, P.sigma, tc + 1, tc + 2, cf, cjv, W, P.tq_half, true, out, out);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) hs[(c * nt + tr) * HC + tc] = out[c].x[0];
+    }
+    __syncthreads();
+    RTile<HC> ht{hs, nt};
+    for (int idx = tid; idx < 2 * nt * TI; idx += 256) {
+        int tc = idx % TI, rest = idx / TI;
+        ss[rest * TI + tc] = hs[rest * HC + tc + 1] + hs[rest * HC + tc];
+    }
+    mbar_wait(&bar[1], 0);
+    __syncthreads();
+    RTile<TI> st2{ss, nt};
+    for (int idx = tid; idx < nt * TI; idx += 256) {
+        int tr = idx / TI, tc = idx - tr * TI;
+        int i = i0 + tc, j = tr;
+        if (i >= nr) continue;
+        R1 out[4];
+        if (i == 0 || i == nr - 1) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) out[c].x[0] = 0.0;
+        } else {
+            R1 bs[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) bs[c] = ut.get(c, j, tc + 2);
+            R1 cjv;
+            cjv.x[0] = __ldg(P.cj + j);
+            RcCoef cf;
+            rc_eval(cf, isi[tr * TI + tc], rti + tc, TI, __ldg(Q.th + j), __ldg(Q.th + nt + j), __ldg(Q.th + 2 * nt + j));
+            substep_wide<1>(ht, st2, tc, j, nt, P.sigma, tc, tc + 1, cf, cjv, W, P.tq_full, false, bs, out);
+        }
+        long g = (long)j * P.pitch + i;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) P.u_out[(long)c * P.plane + g] = out[c].x[0];
+        if (P.obs_raw != nullptr) {
+            int di = i - P.oi, dj = j - P.oj;
+            if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
+                long ks = *P.step_base + P.step_off;
+                if (ks < P.obs_cap) {
+                    double* o = P.obs_raw + ((ks * 4 + (dj * 2 + di)) * 4);
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) o[c] = out[c].x[0];
+                }
+            }
+        }
+    }
+}
+
 // test hook: recomputed folded coefficients of one family written as 8 planes [n_theta][pitch]
 __global__ void rc_tables_kernel(const double* __restrict__ isig, const double* __restrict__ rt, const double* __restrict__ th,
                                  int cols, int n_theta, int pitch, long plane, double* __restrict__ out) {

@@ -78,7 +78,7 @@ struct teuk_ctx {
     int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0, theta_order = 2;
     ThetaWeights tw;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
-    bool use_tma = false, use_rc = false;
+    bool use_tma = false, use_rc = false, use_col_tma = false;
     CUtensorMap tm_state[2], tm_ch, tm_ci, tm_ish, tm_isi, tm_rth, tm_rti;
     // geometry
     int ti = 0, tj = 0, threads = 256;
@@ -412,6 +412,27 @@ template <int TI, int TJ> static bool setup_rc(teuk_ctx* c) {
     return true;
 }
 
+template <int TI> static bool setup_col_tma(teuk_ctx* c) {
+    using G = ColGeom<TI>;
+    const Layout& y = c->lay;
+    const int nt = c->n_theta;
+    double* is0 = c->dptr(y.rc_isig);
+    double* rt0 = c->dptr(y.rc_rt);
+    bool ok = make_map(&c->tm_state[0], c->state(0), c->n_r, nt, 4, y.pitch, y.plane, G::UC, nt, 4) &&
+              make_map(&c->tm_state[1], c->state(1), c->n_r, nt, 4, y.pitch, y.plane, G::UC, nt, 4) &&
+              make_map(&c->tm_isi, is0, c->n_r, nt, 1, y.pitch, y.plane, TI, nt, 1) &&
+              make_map(&c->tm_ish, is0 + y.plane, c->n_r - 1, nt, 1, y.pitch, y.plane, G::CC, nt, 1) &&
+              make_map(&c->tm_rti, rt0, c->n_r, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, TI, RC_NT, 1) &&
+              make_map(&c->tm_rth, rt0 + (size_t)RC_NT * y.pitch, c->n_r - 1, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, G::CC, RC_NT, 1);
+    size_t sm = G::total(nt);
+    if (!ok || sm > 227 * 1024) return false;
+    if (cudaFuncSetAttribute(step_kernel_f64_col_tma<TI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
+        return false;
+    c->ti = TI; c->tj = nt; c->smem = sm; c->threads = 256;
+    c->grid = dim3((c->n_r + TI - 1) / TI, 1);
+    return true;
+}
+
 static const void* col_fn(const teuk_ctx* c, int* threads) {
     *threads = 256;
     if (c->L == 1) return (const void*)step_kernel_col<1, 256, 2>;
@@ -440,8 +461,15 @@ static int choose_geometry(teuk_ctx* c) {
     c->use_tma = false;
     c->use_rc = false;
     if (c->theta_order == 10) {
-        if (c->coef_variant != 0) return TEUK_EINVAL;
         fill_theta_weights(c->tw);
+        c->use_col_tma = false;
+        if (c->L == 1 && c->opt_tma && c->n_theta <= 256 && (c->opt_ti == 0 || c->opt_ti == 8 || c->opt_ti == 12 || c->opt_ti == 16)) {
+            // fp64: TMA column kernel with the semi-recompute coefficient supply (always, whatever coef_variant says)
+            bool ok = c->opt_ti == 16 ? setup_col_tma<16>(c) : c->opt_ti == 12 ? setup_col_tma<12>(c) : setup_col_tma<8>(c);
+            cudaGetLastError();
+            if (ok) { c->use_col_tma = true; return TEUK_OK; }
+        }
+        if (c->coef_variant != 0) return TEUK_EINVAL;
         int ti = c->opt_ti;
         if (ti == 0) {
             // largest tile within the shared-memory budget: 3 blocks/SM for qd (72 KB each), 2 blocks/SM otherwise (100 KB)
@@ -507,7 +535,13 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
     P.obs_cap = c->obs_cap;
     P.step_off = step_off;
     P.oi = c->oi; P.oj = c->oj;
-    if (c->theta_order == 10) {
+    if (c->theta_order == 10 && c->use_col_tma) {
+        RcParams Q{c->dptr(c->lay.rc_th)};
+        const CUtensorMap& tu = c->tm_state[from];
+        if (c->ti == 16) step_kernel_f64_col_tma<16><<<c->grid, 256, c->smem, c->stream>>>(tu, c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q, c->tw);
+        else if (c->ti == 12) step_kernel_f64_col_tma<12><<<c->grid, 256, c->smem, c->stream>>>(tu, c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q, c->tw);
+        else step_kernel_f64_col_tma<8><<<c->grid, 256, c->smem, c->stream>>>(tu, c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q, c->tw);
+    } else if (c->theta_order == 10) {
         void* args[] = {&P, &c->tw};
         int threads = 256;
         const void* fn = col_fn(c, &threads);

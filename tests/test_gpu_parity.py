@@ -229,6 +229,27 @@ def test_theta10_parity_all_precisions(teuk, L, n_r, n_t, steps, base):
     assert not np.array_equal(g2.read(), g.read())
 
 
+@pytest.mark.parametrize("n_r,n_t", [(203, 13), (300, 64), (64, 5), (1000, 70)])
+def test_theta10_fp64_tma_column_kernel(teuk, n_r, n_t):
+    """fp64 theta_order=10 defaults to the TMA column kernel (semi-recompute supply); all its tile widths and the
+    generic column kernel must agree with the oracle"""
+    w = inputs.config(2).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0)
+    w = w.scaled(dt_override=0.5 * inputs.stable_dt(w))
+    u0 = inputs.random_state(n_r, n_t, 1, seed=77)
+    o = oracle.Oracle.from_workload(w, theta_order=10)
+    o.set_observer(10.3, 1.1, 80)
+    o.set_initial(u0)
+    o.step(80)
+    ref, sref = o.read(), o.observe(80)
+    for opts in ({}, {"tile_i": 12}, {"tile_i": 16}, {"use_tma": 0}):
+        g = run_gpu(teuk, w, u0, 80, observer=(10.3, 1.1), options={"theta_order": 10, **opts})
+        geom = g.step_geometry()
+        assert geom["tile_j"] == n_t
+        err = oracle.rel_linf(g.read(), ref)
+        serr = series_err(g.observe(80), sref)
+        assert max(err.values()) <= TOL[1] and max(serr.values()) <= TOL[1], (opts, err, serr)
+
+
 def test_theta10_invariants_and_tiles(teuk):
     w = inputs.config(1).scaled(n_r=96, precision=2)
     u0 = inputs.initial_state(w)
