@@ -230,6 +230,43 @@ def fd_weight_limbs(order):
     return cl, dl
 
 
+# ----------------------------------------------------------------------------- multipole projection (NEXT-2)
+def swsh(s, l, m, theta):
+    """Spin-weighted spherical harmonic _sY_lm(theta, phi = 0) (Goldberg et al. 1967 closed form),
+    written with sin/cos of theta/2 so that the poles are regular:
+      _sY_lm = (-1)^m sqrt[(l+m)!(l-m)!(2l+1) / (4 pi (l+s)!(l-s)!)]
+               * sum_r C(l-s, r) C(l+s, r+s-m) (-1)^(l-r-s) sin^(2l-2r-s+m)(theta/2) cos^(2r+s-m)(theta/2)."""
+    if l < max(abs(s), abs(m)):
+        return mp.mpf(0)
+    pref = (-1) ** m * mp.sqrt(mp.factorial(l + m) * mp.factorial(l - m) * (2 * l + 1)
+                               / (4 * mp.pi * mp.factorial(l + s) * mp.factorial(l - s)))
+    sh, ch = mp.sin(theta / 2), mp.cos(theta / 2)
+    tot = mp.mpf(0)
+    for r in range(0, l - s + 1):
+        k = r + s - m
+        if k < 0 or k > l + s:
+            continue
+        tot += mp.binomial(l - s, r) * mp.binomial(l + s, k) * (-1) ** (l - r - s) * sh ** (2 * l - 2 * r - s + m) * ch ** (2 * r + s - m)
+    return pref * tot
+
+
+def multipole_weights(s, m, n_theta, n_ell):
+    """Q[k][j] = 2 pi dtheta sin(theta_j) _sY_{l_min+k, m}(theta_j): midpoint-rule weights of the projection
+         a_l'(t) = int Phi(t, r*_obs, theta) conj(_sY_l'm) dOmega      (Fig. 1; reading A24)
+    on the cell-centred theta grid, l_min = max(|s|, |m|).  Returns quad-double limbs [n_ell][n_theta][4]."""
+    with mp.workdps(MP_DPS):
+        dth = mp.pi / n_theta
+        lmin = max(abs(s), abs(m))
+        out = []
+        for k in range(n_ell):
+            row = []
+            for j in range(n_theta):
+                th = (j + mp.mpf(1) / 2) * dth
+                row.append(to_limbs(2 * mp.pi * dth * mp.sin(th) * swsh(s, lmin + k, m, th)))
+            out.append(row)
+        return out
+
+
 # ----------------------------------------------------------------------------- Eqs. (13)-(14)
 class MPStepper:
     """Literal mpmath implementation of one Lax-Wendroff iteration on a tiny

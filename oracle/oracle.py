@@ -52,6 +52,8 @@ def lib():
         _lib.oracle_set_tables.argtypes = [C.c_void_p, C.c_int, dp]
         _lib.oracle_get_cot.argtypes = [C.c_void_p, dp]
         _lib.oracle_lambda.argtypes = [C.c_void_p, dp, dp]
+        _lib.oracle_set_multipole.argtypes = [C.c_void_p, C.c_double, C.c_int, dp, C.c_long]
+        _lib.oracle_observe_multipoles.argtypes = [C.c_void_p, dp, C.c_long, C.POINTER(C.c_long)]
         _lib.oracle_destroy.argtypes = [C.c_void_p]
         _lib.oracle_destroy.restype = None
         _lib.oracle_mp_op.argtypes = [C.c_int, C.c_int, dp, dp, dp]
@@ -89,6 +91,7 @@ class Oracle:
                  theta_order=2):
         self.n_win = n_r - i_lo if n_win is None else n_win
         self.n_r, self.n_theta, self.L, self.i_lo = n_r, n_theta, precision, i_lo
+        self.s, self.m = s, m
         key = (float(M), float(a), float(rstar_min), float(rstar_max), n_r, i_lo, self.n_win)
         if key not in _table_cache:
             _table_cache[key] = mp_ref.radial_tables(M, a, rstar_min, rstar_max, n_r, i_lo, self.n_win)
@@ -120,6 +123,19 @@ class Oracle:
 
     def set_observer(self, rstar_obs, theta_obs, capacity):
         self._chk(lib().oracle_set_observer(self.h, rstar_obs, theta_obs, capacity))
+
+    def set_multipole_observer(self, rstar_obs, n_ell, capacity):
+        """NEXT-2: per step, project Phi(r*_obs, theta) on _sY_l'm, l' = l_min .. l_min + n_ell - 1 (reading A24)."""
+        q = np.ascontiguousarray(np.array(mp_ref.multipole_weights(self.s, self.m, self.n_theta, n_ell), dtype=np.float64))
+        self._mpq, self.n_ell = q, n_ell
+        self._chk(lib().oracle_set_multipole(self.h, rstar_obs, n_ell, _dp(q), capacity))
+
+    def observe_multipoles(self, max_samples: int) -> np.ndarray:
+        """[count][n_ell][2][L]: real and imaginary part of a_l' after each completed step"""
+        out = np.zeros((max(max_samples, 1), self.n_ell, 2, self.L))
+        cnt = C.c_long(0)
+        self._chk(lib().oracle_observe_multipoles(self.h, _dp(out), max_samples, C.byref(cnt)))
+        return out[:cnt.value]
 
     def set_initial(self, planes: np.ndarray):
         """planes: [4][N_theta][N_win] (fp64, low limbs := 0) or [4][L][N_theta][N_win]."""

@@ -89,6 +89,8 @@ struct Base {
     virtual int tables(int half, double* out, const double* in) = 0;
     virtual int cot_table(double* out) = 0;
     virtual int lambda(const double* f, double* out) = 0;
+    virtual int set_multipole(double ro, int n_ell, const double* q_l, long cap) = 0;
+    virtual int observe_multipoles(double* out, long maxs, long* count) = 0;
     long steps_done = 0;
 };
 
@@ -109,6 +111,12 @@ struct Solver : Base {
     int oi = -1, oj = -1;
     T wr, wt;
     std::vector<T> series;                // [sample][4]
+    // multipole-projection observer (NEXT-2; Fig. 1; reading A24)
+    long mp_cap = 0;
+    int mp_n = 0, mp_i = -1;
+    T mp_wr;
+    std::vector<T> mp_q;                  // [n_ell][n_theta]
+    std::vector<T> mp_series;             // [sample][n_ell][2]
 
     int build(const double* r_tab, const double* d_tab, const double* sin_tab, const double* cos_tab,
               const double* dr_l, const double* dth_l, const double* wc_l, const double* wd_l) override {
@@ -178,6 +186,32 @@ struct Solver : Base {
         return OK;
     }
 
+    int set_multipole(double ro, int n_ell, const double* q_l, long cap) override {
+        if (cap < 0 || n_ell < 1 || n_ell > 32) return EINVAL;
+        Q x = (Q(ro) - Q(P.rmin)) / dr_q;
+        int i0 = (int)std::floor(x.x[0]);
+        if (i0 < 0 || x.x[0] > P.n_r - 1) return EINVAL;
+        if (i0 > P.n_r - 2) i0 = P.n_r - 2;
+        mp_wr = narrow<T>(x - Q((double)i0));
+        mp_i = i0 - P.i_lo;
+        if (mp_i < 0 || mp_i + 1 >= P.n_win) return EINVAL;
+        mp_n = n_ell;
+        mp_q.resize((size_t)n_ell * P.n_theta);
+        for (size_t k = 0; k < mp_q.size(); ++k) mp_q[k] = narrow<T>(Q::from_limbs(q_l + 4 * k, 4));
+        mp_cap = cap;
+        mp_series.clear();
+        return OK;
+    }
+
+    int observe_multipoles(double* out, long maxs, long* count) override {
+        long n = mp_n ? (long)(mp_series.size() / (2 * mp_n)) : 0;
+        if (n > maxs) n = maxs;
+        for (size_t q = 0; q < (size_t)n * mp_n * 2; ++q)
+            for (int k = 0; k < L; ++k) out[q * L + k] = Limbs<T>::get(mp_series[q], k);
+        *count = n;
+        return OK;
+    }
+
     int set_initial(const double* planes, int limbs_in) override {
         if (limbs_in != 1 && limbs_in != L) return EINVAL;
         const int nw = P.n_win, nt = P.n_theta;
@@ -193,6 +227,7 @@ struct Solver : Base {
         have_init = true;
         steps_done = 0;
         series.clear();
+        mp_series.clear();
         return OK;
     }
 
@@ -305,6 +340,19 @@ struct Solver : Base {
                 u[f].swap(un[f]);
             }
             ++steps_done;
+            if (mp_cap > 0 && (long)(mp_series.size() / (2 * mp_n)) < mp_cap) {
+                // a_l' = sum_j Q_l'(theta_j) [ (1 - w) Phi(i0, j) + w Phi(i0 + 1, j) ],  j = 0 .. N_theta - 1 in order
+                T one(1.0);
+                for (int k = 0; k < mp_n; ++k)
+                    for (int c = 0; c < 2; ++c) {
+                        T acc(0.0);
+                        for (int j = 0; j < nt; ++j) {
+                            T v = (one - mp_wr) * u[c][(size_t)mp_i * nt + j] + mp_wr * u[c][(size_t)(mp_i + 1) * nt + j];
+                            acc = acc + mp_q[(size_t)k * nt + j] * v;
+                        }
+                        mp_series.push_back(acc);
+                    }
+            }
             if (obs_cap > 0 && (long)(series.size() / 4) < obs_cap) {   // O7
                 T one(1.0);
                 for (int f = 0; f < 4; ++f) {
@@ -429,6 +477,8 @@ int oracle_get_tables(void* h, int half, double* out) { return ((Base*)h)->table
 int oracle_set_tables(void* h, int half, const double* in) { return ((Base*)h)->tables(half, nullptr, in); }
 int oracle_get_cot(void* h, double* out) { return ((Base*)h)->cot_table(out); }
 int oracle_lambda(void* h, const double* f, double* out) { return ((Base*)h)->lambda(f, out); }
+int oracle_set_multipole(void* h, double ro, int n_ell, const double* q_l, long cap) { return ((Base*)h)->set_multipole(ro, n_ell, q_l, cap); }
+int oracle_observe_multipoles(void* h, double* out, long maxs, long* count) { return ((Base*)h)->observe_multipoles(out, maxs, count); }
 int oracle_steps_done(void* h, long* n) { *n = ((Base*)h)->steps_done; return OK; }
 void oracle_destroy(void* h) { delete (Base*)h; }
 int oracle_set_threads(int n) {
