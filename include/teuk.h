@@ -73,6 +73,15 @@ int teuk_read_device(teuk_ctx *, double *d_planes);
  * TEUK_ENONFINITE (sticky, data still written) if any recorded sample was not finite. */
 int teuk_observe(teuk_ctx *, double *host_out, long max_samples, long *count);
 
+/* Multipole-projection observer (the paper's Fig. 1 workload): after every iteration,
+ * a_l' = integral of Phi(r*_obs, theta) _sY_l'm(theta) over the sphere, l' = l_min .. l_min + n_ell - 1 with
+ * l_min = max(|s|, |m|), 1 <= n_ell <= 9, Fejer's first quadrature rule on the cell-centred theta grid (exact for
+ * polynomials of degree < n_theta in cos(theta)), linear interpolation in r*.
+ * capacity <= obs_capacity of teuk_create.  Call before teuk_set_initial or between teuk_step calls. */
+int teuk_set_multipole_observer(teuk_ctx *, double rstar_obs, int n_ell, long capacity);
+/* host_out[count][n_ell][2][L]: real and imaginary part of a_l' per completed iteration; synchronises. */
+int teuk_observe_multipoles(teuk_ctx *, double *host_out, long max_samples, long *count);
+
 int teuk_steps_done(teuk_ctx *, long *n);
 /* Number of kernels this handle has launched so far (graph nodes counted per replay). */
 int teuk_launch_count(teuk_ctx *, long *n);

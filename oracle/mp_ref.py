@@ -250,19 +250,37 @@ def swsh(s, l, m, theta):
     return pref * tot
 
 
+def fejer_weights(n_theta):
+    """Fejer's first quadrature rule: nodes x_j = cos(theta_j) with theta_j = (j + 1/2) pi / N are exactly the
+    cell-centred theta grid, and  int_0^pi F(theta) sin(theta) dtheta ~ sum_j w_j F(theta_j),
+        w_j = (2/N) [1 - 2 sum_{k=1}^{floor(N/2)} cos(2 k theta_j) / (4 k^2 - 1)],
+    exact when F is a polynomial of degree < N in cos(theta) (spectrally accurate, unlike the midpoint rule whose
+    O(dtheta^2) error would leak the dominant multipole into every other one)."""
+    N = n_theta
+    out = []
+    for j in range(N):
+        th = (j + mp.mpf(1) / 2) * mp.pi / N
+        acc = mp.mpf(1)
+        for k in range(1, N // 2 + 1):
+            acc -= 2 * mp.cos(2 * k * th) / (4 * k * k - 1)
+        out.append(2 * acc / N)
+    return out
+
+
 def multipole_weights(s, m, n_theta, n_ell):
-    """Q[k][j] = 2 pi dtheta sin(theta_j) _sY_{l_min+k, m}(theta_j): midpoint-rule weights of the projection
+    """Q[k][j] = 2 pi w_j _sY_{l_min+k, m}(theta_j), w_j = Fejer-1 weights: the projection
          a_l'(t) = int Phi(t, r*_obs, theta) conj(_sY_l'm) dOmega      (Fig. 1; reading A24)
     on the cell-centred theta grid, l_min = max(|s|, |m|).  Returns quad-double limbs [n_ell][n_theta][4]."""
     with mp.workdps(MP_DPS):
         dth = mp.pi / n_theta
         lmin = max(abs(s), abs(m))
+        wf = fejer_weights(n_theta)
         out = []
         for k in range(n_ell):
             row = []
             for j in range(n_theta):
                 th = (j + mp.mpf(1) / 2) * dth
-                row.append(to_limbs(2 * mp.pi * dth * mp.sin(th) * swsh(s, lmin + k, m, th)))
+                row.append(to_limbs(2 * mp.pi * wf[j] * swsh(s, lmin + k, m, th)))
             out.append(row)
         return out
 

@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <algorithm>
 #include <cstring>
 #include <vector>
 
@@ -29,11 +30,12 @@ static int cuda_fail(cudaError_t e, const char* what, int line) {
     } while (0)
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+constexpr int MP_MAX_ELL = 9;      // l' = l_min .. l_min + 8 (Fig. 1)
 
 struct Layout {
     int pitch;
     long plane;
-    size_t state_a, state_b, coef_i, coef_h, cj, r_tab, d_tab, sin_tab, cos_tab, obs_raw, obs_out, scalars, rc_rt, rc_isig, rc_th, total;
+    size_t state_a, state_b, coef_i, coef_h, cj, r_tab, d_tab, sin_tab, cos_tab, obs_raw, obs_out, scalars, rc_rt, rc_isig, rc_th, mp_q, mp_series, total;
 };
 
 static Layout make_layout(int n_r, int n_theta, int L, long cap) {
@@ -62,6 +64,9 @@ static Layout make_layout(int n_r, int n_theta, int L, long cap) {
     y.rc_rt = take(L == 1 ? (size_t)2 * RC_NT * y.pitch : 1);
     y.rc_isig = take(L == 1 ? (size_t)2 * y.plane : 1);
     y.rc_th = take(L == 1 ? (size_t)3 * n_theta : 1);
+    // multipole-projection observer (NEXT-2): weights [9][L][n_theta], series [cap][9][2][L]
+    y.mp_q = take((size_t)MP_MAX_ELL * L * n_theta);
+    y.mp_series = take((size_t)(cap > 0 ? cap : 1) * MP_MAX_ELL * 2 * L);
     y.total = off;
     return y;
 }
@@ -93,6 +98,10 @@ struct teuk_ctx {
     int oi = 0, oj = 0;
     R4 wr, wt;
     bool nonfinite = false;
+    // multipole-projection observer
+    long mp_cap = 0;
+    int mp_n = 0, mp_i = 0;
+    R4 mp_wr;
     cudaGraphExec_t graph[2] = {nullptr, nullptr};
 
     double* dptr(size_t off) const { return (double*)(ws + off); }
@@ -128,6 +137,55 @@ __global__ void observer_combine_kernel(const double* __restrict__ raw, double* 
         bad |= !isfinite(v.x[l]);
     }
     if (bad) atomicOr(flag, 1);
+}
+
+// NEXT-2 (Fig. 1; reading A24): a_l' = sum_j Q_l'(theta_j) [(1-w) Phi(i0,j) + w Phi(i0+1,j)]
+// for l' = l_min .. l_min + n_ell - 1, real and imaginary part, once per step.  One block of 32 x 2 n_ell threads:
+// the interpolated column is staged in shared memory, one warp per output does a strided sum + shuffle tree.
+template <int L>
+__global__ void multipole_kernel(const double* __restrict__ u, const double* __restrict__ q, double* __restrict__ series,
+                                 const long* step_base, int step_off, long cap, int n_ell, int nt, int pitch, long plane,
+                                 int i0, R4 wr) {
+    extern __shared__ double v[];                 // [2][L][nt]
+    const int tid = threadIdx.x, nth = blockDim.x;
+    const Real<L> w = narrow<L>(wr), omw = sub(from_double<L>(1.0), narrow<L>(wr));
+    for (int idx = tid; idx < 2 * nt; idx += nth) {
+        int c = idx / nt, j = idx - c * nt;
+        Real<L> a, b;
+#pragma unroll
+        for (int l = 0; l < L; ++l) {
+            a.x[l] = u[(long)(c * L + l) * plane + (long)j * pitch + i0];
+            b.x[l] = u[(long)(c * L + l) * plane + (long)j * pitch + i0 + 1];
+        }
+        Real<L> val = add(mul(omw, a), mul(w, b));
+#pragma unroll
+        for (int l = 0; l < L; ++l) v[(c * L + l) * nt + j] = val.x[l];
+    }
+    __syncthreads();
+    const int warp = tid >> 5, lane = tid & 31;
+    if (warp >= 2 * n_ell) return;
+    const int k = warp >> 1, c = warp & 1;
+    Real<L> acc = from_double<L>(0.0);
+    for (int j = lane; j < nt; j += 32) {
+        Real<L> qq, vv;
+#pragma unroll
+        for (int l = 0; l < L; ++l) { qq.x[l] = q[(long)(k * L + l) * nt + j]; vv.x[l] = v[(c * L + l) * nt + j]; }
+        acc = add(acc, mul(qq, vv));
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        Real<L> o;
+#pragma unroll
+        for (int l = 0; l < L; ++l) o.x[l] = __shfl_down_sync(0xffffffffu, acc.x[l], off);
+        acc = add(acc, o);
+    }
+    if (lane == 0) {
+        long smp = *step_base + step_off;
+        if (smp < cap) {
+#pragma unroll
+            for (int l = 0; l < L; ++l) series[((smp * n_ell + k) * 2 + c) * L + l] = acc.x[l];
+        }
+    }
 }
 
 // set_initial on the device: copy limbs_in planes per field into L planes (missing limbs := 0), force the
@@ -559,6 +617,16 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         const void* fn = step_fn(c, &threads);
         if (cudaLaunchKernel(fn, c->grid, dim3(threads), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
     }
+    if (c->mp_cap > 0) {
+        const double* uo = c->state(from ^ 1);
+        const double* qd_ = c->dptr(c->lay.mp_q);
+        double* ser = c->dptr(c->lay.mp_series);
+        int threads = 64 * c->mp_n;
+        size_t sm = (size_t)2 * c->L * c->n_theta * sizeof(double);
+        if (c->L == 1) multipole_kernel<1><<<1, threads, sm, c->stream>>>(uo, qd_, ser, c->step_base(), step_off, c->mp_cap, c->mp_n, c->n_theta, c->lay.pitch, c->lay.plane, c->mp_i, c->mp_wr);
+        else if (c->L == 2) multipole_kernel<2><<<1, threads, sm, c->stream>>>(uo, qd_, ser, c->step_base(), step_off, c->mp_cap, c->mp_n, c->n_theta, c->lay.pitch, c->lay.plane, c->mp_i, c->mp_wr);
+        else multipole_kernel<4><<<1, threads, sm, c->stream>>>(uo, qd_, ser, c->step_base(), step_off, c->mp_cap, c->mp_n, c->n_theta, c->lay.pitch, c->lay.plane, c->mp_i, c->mp_wr);
+    }
     return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
 }
 
@@ -622,7 +690,7 @@ extern "C" int teuk_step(teuk_ctx* c, long n) {
             if (rc != TEUK_OK) return rc;
         }
         CK(cudaGraphLaunch(c->graph[c->cur], c->stream));
-        c->launches += K + 1;
+        c->launches += (c->mp_cap > 0 ? 2 * K : K) + 1;
         left -= K;                            // K is even: c->cur unchanged
     }
     if (left > 0) {
@@ -632,7 +700,7 @@ extern "C" int teuk_step(teuk_ctx* c, long n) {
             c->cur ^= 1;
         }
         advance_kernel<<<1, 1, 0, c->stream>>>(c->step_base(), left);
-        c->launches += left + 1;
+        c->launches += (c->mp_cap > 0 ? 2 * left : left) + 1;
         if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
     }
     c->steps_done += n;
@@ -685,6 +753,105 @@ extern "C" int teuk_observe(teuk_ctx* c, double* host_out, long max_samples, lon
     }
     *count = n;
     return c->nonfinite ? TEUK_ENONFINITE : TEUK_OK;
+}
+
+// ---- NEXT-2: multipole-projection observer ------------------------------------------------------------------
+static R4 q_factorial(int n) {
+    R4 r = from_double<4>(1.0);
+    for (int k = 2; k <= n; ++k) r = mul_d(r, (double)k);
+    return r;
+}
+static double binom_d(int n, int k) {          // exact in fp64 for the small arguments used here (n <= 40)
+    if (k < 0 || k > n) return 0.0;
+    double r = 1.0;
+    for (int i = 1; i <= k; ++i) r = r * (double)(n - k + i) / (double)i;
+    return nearbyint(r);
+}
+static R4 q_powi(const R4& x, int n) {
+    R4 r = from_double<4>(1.0);
+    for (int i = 0; i < n; ++i) r = mul(r, x);
+    return r;
+}
+// _sY_lm(theta, 0) from the Goldberg closed form written in sin, cos of theta/2 (regular at the poles)
+static R4 q_swsh(int s, int l, int m, const R4& sh, const R4& ch, const R4& pi) {
+    R4 num = mul_d(mul(q_factorial(l + m), q_factorial(l - m)), (double)(2 * l + 1));
+    R4 den = mul(scale2(pi, 4.0), mul(q_factorial(l + s), q_factorial(l - s)));
+    R4 pref = msqrt(div(num, den));
+    if (m & 1) pref = neg(pref);
+    R4 tot = from_double<4>(0.0);
+    for (int r = 0; r <= l - s; ++r) {
+        int k = r + s - m;
+        if (k < 0 || k > l + s) continue;
+        double cf = binom_d(l - s, r) * binom_d(l + s, k) * (((l - r - s) & 1) ? -1.0 : 1.0);
+        tot = add(tot, mul_d(mul(q_powi(sh, 2 * l - 2 * r - s + m), q_powi(ch, 2 * r + s - m)), cf));
+    }
+    return mul(pref, tot);
+}
+
+// cos(pi p / N) for integers p, N in quad-double: the angle is reduced to [0, pi/2] with integer arithmetic first
+static R4 q_cos_pi_frac(long p, long N, const R4& pi) {
+    p %= 2 * N;
+    if (p < 0) p += 2 * N;
+    if (p > N) p = 2 * N - p;                  // cos(2 pi - x) = cos x
+    bool negate = false;
+    if (2 * p > N) { p = N - p; negate = true; }   // cos(pi - x) = -cos x
+    R4 sn, cs;
+    q_sincos(div(mul_d(pi, (double)p), from_double<4>((double)N)), sn, cs);
+    return negate ? neg(cs) : cs;
+}
+// Fejer's first rule on the cell-centred grid: w_j = (2/N) [1 - 2 sum_{k=1}^{N/2} cos(2 k theta_j) / (4 k^2 - 1)];
+// exact for polynomials of degree < N in cos(theta), so the dominant multipole does not leak into the others.
+static R4 q_fejer_weight(int j, int N, const R4& pi) {
+    R4 acc = from_double<4>(1.0);
+    for (long k = 1; k <= N / 2; ++k) {
+        R4 ck = q_cos_pi_frac(k * (2L * j + 1), N, pi);           // 2 k theta_j = pi k (2j + 1) / N
+        acc = sub(acc, div(scale2(ck, 2.0), from_double<4>((double)(4 * k * k - 1))));
+    }
+    return div(scale2(acc, 2.0), from_double<4>((double)N));
+}
+
+extern "C" int teuk_set_multipole_observer(teuk_ctx* c, double rstar_obs, int n_ell, long capacity) {
+    if (!c || n_ell < 1 || n_ell > MP_MAX_ELL || capacity < 0 || capacity > c->cap_alloc || !std::isfinite(rstar_obs))
+        return TEUK_EINVAL;
+    R4 x = div(sub(from_double<4>(rstar_obs), c->C.rmin), c->C.dr);
+    int i0 = (int)std::floor(x.x[0]);
+    if (x.x[0] < 0 || x.x[0] > c->n_r - 1) return TEUK_EINVAL;
+    if (i0 > c->n_r - 2) i0 = c->n_r - 2;
+    c->mp_wr = sub(x, from_double<4>((double)i0));
+    c->mp_i = i0; c->mp_n = n_ell; c->mp_cap = capacity;
+    // weights Q_k(theta_j) = 2 pi w_j _sY_{l_min + k, m}(theta_j), w_j = Fejer-1 weights, in quad-double on the host
+    QConst qc = q_constants();
+    const int nt = c->n_theta, L = c->L;
+    const int lmin = std::max(std::abs(c->s), std::abs(c->m));
+    std::vector<double> q((size_t)MP_MAX_ELL * L * nt, 0.0);
+    R4 two_pi = scale2(qc.pi, 2.0);
+    for (int j = 0; j < nt; ++j) {
+        R4 th = mul(c->C.dth, add(from_double<4>((double)j), from_double<4>(0.5)));
+        R4 sh, ch;
+        q_sincos(scale2(th, 0.5), sh, ch);
+        R4 wf = mul(two_pi, q_fejer_weight(j, nt, qc.pi));
+        for (int k = 0; k < n_ell; ++k) {
+            R4 w = mul(wf, q_swsh(c->s, lmin + k, c->m, sh, ch, qc.pi));
+            for (int l = 0; l < L; ++l) q[((size_t)k * L + l) * nt + j] = w.x[l];
+        }
+    }
+    for (int p = 0; p < 2; ++p)
+        if (c->graph[p]) { cudaGraphExecDestroy(c->graph[p]); c->graph[p] = nullptr; }
+    CK(cudaMemcpyAsync(c->dptr(c->lay.mp_q), q.data(), q.size() * 8, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return TEUK_OK;
+}
+
+extern "C" int teuk_observe_multipoles(teuk_ctx* c, double* host_out, long max_samples, long* count) {
+    if (!c || !host_out || !count || max_samples < 0) return TEUK_EINVAL;
+    long n = c->steps_done < c->mp_cap ? c->steps_done : c->mp_cap;
+    if (n > max_samples) n = max_samples;
+    if (n > 0)
+        CK(cudaMemcpyAsync(host_out, c->dptr(c->lay.mp_series), (size_t)n * c->mp_n * 2 * c->L * sizeof(double),
+                           cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    *count = n;
+    return TEUK_OK;
 }
 
 extern "C" int teuk_steps_done(teuk_ctx* c, long* n) {

@@ -35,6 +35,8 @@ SIGNATURES = {
     "teuk_read": (C.c_int, [_h, _dp]),
     "teuk_read_device": (C.c_int, [_h, C.c_void_p]),
     "teuk_observe": (C.c_int, [_h, _dp, C.c_long, _lp]),
+    "teuk_set_multipole_observer": (C.c_int, [_h, C.c_double, C.c_int, C.c_long]),
+    "teuk_observe_multipoles": (C.c_int, [_h, _dp, C.c_long, _lp]),
     "teuk_steps_done": (C.c_int, [_h, _lp]),
     "teuk_launch_count": (C.c_int, [_h, _lp]),
     "teuk_step_geometry": (C.c_int, [_h, _lp]),
@@ -105,7 +107,7 @@ class Teuk:
                    precision or w.precision, obs_capacity, **kw)
 
     def close(self):
-        if getattr(self, "h", None):
+        if getattr(self, "h", None) and lib is not None:
             lib.teuk_destroy(self.h)
             self.h = None
 
@@ -163,6 +165,16 @@ class Teuk:
         rc = _chk(lib.teuk_observe(self.h, _np(out), max_samples, C.byref(cnt)), "teuk_observe",
                   allow=(ENONFINITE,) if allow_nonfinite else ())
         self.last_observe_status = rc
+        return out[:cnt.value]
+
+    def set_multipole_observer(self, rstar_obs, n_ell, capacity):
+        self.n_ell = n_ell
+        _chk(lib.teuk_set_multipole_observer(self.h, rstar_obs, n_ell, capacity), "teuk_set_multipole_observer")
+
+    def observe_multipoles(self, max_samples: int) -> np.ndarray:
+        out = np.zeros((max(max_samples, 1), self.n_ell, 2, self.L))
+        cnt = C.c_long(0)
+        _chk(lib.teuk_observe_multipoles(self.h, _np(out), max_samples, C.byref(cnt)), "teuk_observe_multipoles")
         return out[:cnt.value]
 
     def steps_done(self) -> int:

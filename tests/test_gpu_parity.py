@@ -292,6 +292,72 @@ def test_theta10_full_size_configs_windowed(teuk, cfg, steps_gpu, k):
             assert float(np.hypot(dre, dim).max() / den) <= TOL[L], (cfg, i_lo, re)
 
 
+# ------------------------------------------------------------------------------- NEXT-2: multipole-projection observer
+def _mp_err(a, b):
+    """series [n][n_ell][2][L]: max |a - b| over everything / max |b| (complex), differences formed exactly"""
+    n, ne, _, L = b.shape
+    A = np.ascontiguousarray(np.transpose(a, (2, 3, 0, 1)))      # [2][L][n][n_ell]
+    B = np.ascontiguousarray(np.transpose(b, (2, 3, 0, 1)))
+    dre, _ = oracle._limb_diff(A[0], B[0])
+    dim, _ = oracle._limb_diff(A[1], B[1])
+    return float(np.hypot(dre, dim).max() / np.hypot(B[0, 0], B[1, 0]).max())
+
+
+@pytest.mark.parametrize("L,base,n_r,n_t,steps,order", [(1, 2, 203, 24, 120, 2), (2, 2, 150, 16, 60, 2), (4, 2, 90, 12, 30, 2),
+                                                        (1, 4, 300, 40, 100, 2), (2, 4, 120, 32, 40, 10), (4, 4, 80, 32, 20, 10)])
+def test_multipole_observer_parity(teuk, L, base, n_r, n_t, steps, order):
+    w = inputs.config(base).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0, precision=L)
+    w = w.scaled(dt_override=0.5 * inputs.stable_dt(w))
+    u0 = inputs.random_state(n_r, n_t, L, seed=300 + L)
+    n_ell = 9
+    g = teuk.Teuk.from_workload(w, obs_capacity=steps)
+    g.set_option("theta_order", order)
+    g.set_option("graph_steps", 8)
+    g.set_observer(10.3, 1.1, steps)
+    g.set_multipole_observer(12.7, n_ell, steps)
+    g.set_initial(u0)
+    g.step(steps)
+    o = oracle.Oracle.from_workload(w, theta_order=order)
+    o.set_observer(10.3, 1.1, steps)
+    o.set_multipole_observer(12.7, n_ell, steps)
+    o.set_initial(u0)
+    o.step(steps)
+    got, ref = g.observe_multipoles(steps), o.observe_multipoles(steps)
+    assert got.shape == ref.shape == (steps, n_ell, 2, L)
+    err = _mp_err(got, ref)
+    print("multipoles", L, base, order, err)
+    assert err <= TOL[L]
+    assert max(series_err(g.observe(steps), o.observe(steps)).values()) <= TOL[L]      # the point observer still works beside it
+    assert max(oracle.rel_linf(g.read(), o.read()).values()) <= TOL[L]
+
+
+def test_multipole_observer_config4_full_size(teuk):
+    """config 4 (qd, 8192 x 32, a = 0.5, pure l = 0 data: the Fig. 1 setting) at full size: the oracle advances a radial
+    window around the observer from the GPU's state and must reproduce the projected series"""
+    w = inputs.config(4)
+    u0 = inputs.initial_state(w)
+    k, pre = 5, 40
+    g = teuk.Teuk.from_workload(w, obs_capacity=pre + k)
+    g.set_multipole_observer(w.rstar_obs, 9, pre + k)
+    g.set_initial(u0)
+    g.step(pre)
+    mid = g.read()
+    g.step(k)
+    got = g.observe_multipoles(pre + k)[pre:]
+    i_c = int((w.rstar_obs - w.rstar_min) / w.dr)
+    n_win = 48
+    i_lo = i_c - n_win // 2
+    o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win)
+    o.set_multipole_observer(w.rstar_obs, 9, k)
+    o.set_initial(np.ascontiguousarray(mid[..., i_lo:i_lo + n_win]))
+    o.step(k)
+    err = _mp_err(got, o.observe_multipoles(k))
+    print("cfg4 multipoles, full size:", err)
+    assert err <= TOL[4]
+    with pytest.raises(teuk.TeukError):
+        g.set_multipole_observer(w.rstar_obs, 10, 1)          # at most 9 multipoles (l' = 0..8 of Fig. 1)
+
+
 # ------------------------------------------------------------------------------- full-size configs (bench launch geometry)
 @pytest.mark.parametrize("cfg,steps_gpu,k", [(2, 300, 12), (3, 120, 8), (4, 100, 6)])
 def test_full_size_configs_windowed(teuk, cfg, steps_gpu, k):
