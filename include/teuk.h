@@ -43,7 +43,8 @@ int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double r
  * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic), "use_tma" (fp64: 1 = TMA
  * kernel, default; 0 = generic kernel), "variant" (dd/qd launch shape 0..2), "coef_variant" (0 = precomputed
  * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only),
- * "theta_order" (2 = second-order centred theta differences, default; 10 = the 10th-order
+ * "pdl" (fp64 TMA kernels: 1 = programmatic dependent launch, the next step prefetches its half-step coefficient
+ * tile while the current one drains; default 0, measured neutral), "theta_order" (2 = second-order centred theta differences, default; 10 = the 10th-order
  * 11-point operator of PAPER.md:126, needs n_theta >= 5). */
 int teuk_set_option(teuk_ctx *, const char *key, double value);
 

@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(256) step_kernel_f64_tma(const __grid_constant
     using G = TmaGeom<TI, TJ>;
     constexpr int UC = G::UC, UR = G::UR, HC = G::HC, HR = G::HR, CC = G::CC;
     extern __shared__ __align__(128) unsigned char raw[];
-    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ __align__(8) uint64_t bar[3];
     unsigned char* base = (unsigned char*)(((uintptr_t)raw + 127) & ~(uintptr_t)127);
     double* us = (double*)base;
     double* chs = (double*)(base + G::US_B);
@@ -94,21 +94,29 @@ __global__ void __launch_bounds__(256) step_kernel_f64_tma(const __grid_constant
     const int nt = P.n_theta, nr = P.n_r;
     const int tid = threadIdx.x;
 
+    // Programmatic dependent launch: let the next step's grid start as soon as SM resources free up ...
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (tid == 0) {
         mbar_init(&bar[0], 1);
         mbar_init(&bar[1], 1);
+        mbar_init(&bar[2], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        // ... and fetch the TIME-INDEPENDENT coefficient tiles before waiting for the previous step to finish
+        // (the half-step tile only: the TMA unit serves requests in order, and the full-step tile must not delay u)
+        mbar_expect_tx(&bar[2], 8 * HR * CC * 8);
+        tma_load_3d(chs, &tm_ch, i0 - 2, j0 - 1, 0, &bar[2]);
     }
-    __syncthreads();
+    asm volatile("griddepcontrol.wait;" ::: "memory");        // u^n (written by the previous step) is complete and visible
     if (tid == 0) {
-        mbar_expect_tx(&bar[0], 4 * UR * UC * 8 + 8 * HR * CC * 8);
+        mbar_expect_tx(&bar[0], 4 * UR * UC * 8);
         tma_load_3d(us, &tm_u, i0 - 2, j0 - 2, 0, &bar[0]);
-        tma_load_3d(chs, &tm_ch, i0 - 2, j0 - 1, 0, &bar[0]);
         mbar_expect_tx(&bar[1], 8 * TJ * TI * 8);
         tma_load_3d(cis, &tm_ci, i0, j0, 0, &bar[1]);
     }
+    __syncthreads();
     mbar_wait(&bar[0], 0);
+    mbar_wait(&bar[2], 0);
 
     CTile<UR, UC> ut{us, j0 - 2};
     // ---- half step, Eq. (13)
@@ -231,7 +239,7 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
     using G = RcGeom<TI, TJ>;
     constexpr int UC = G::UC, UR = G::UR, HC = G::HC, HR = G::HR, CC = G::CC, NT = G::NT;
     extern __shared__ __align__(128) unsigned char raw[];
-    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ __align__(8) uint64_t bar[3];
     unsigned char* base = (unsigned char*)(((uintptr_t)raw + 127) & ~(uintptr_t)127);
     double* us = (double*)base;
     double* ish = (double*)(base + G::US_B);
@@ -243,23 +251,28 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
     const int nt = P.n_theta, nr = P.n_r;
     const int tid = threadIdx.x;
 
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (tid == 0) {
         mbar_init(&bar[0], 1);
         mbar_init(&bar[1], 1);
+        mbar_init(&bar[2], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(&bar[2], HR * CC * 8 + NT * CC * 8);
+        tma_load_3d(ish, &tm_ish, i0 - 2, j0 - 1, 0, &bar[2]);
+        tma_load_3d(rth, &tm_rth, i0 - 2, 0, 0, &bar[2]);
     }
-    __syncthreads();
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (tid == 0) {
-        mbar_expect_tx(&bar[0], 4 * UR * UC * 8 + HR * CC * 8 + NT * CC * 8);
+        mbar_expect_tx(&bar[0], 4 * UR * UC * 8);
         tma_load_3d(us, &tm_u, i0 - 2, j0 - 2, 0, &bar[0]);
-        tma_load_3d(ish, &tm_ish, i0 - 2, j0 - 1, 0, &bar[0]);
-        tma_load_3d(rth, &tm_rth, i0 - 2, 0, 0, &bar[0]);
         mbar_expect_tx(&bar[1], TJ * TI * 8 + NT * TI * 8);
         tma_load_3d(isi, &tm_isi, i0, j0, 0, &bar[1]);
         tma_load_3d(rti, &tm_rti, i0, 0, 0, &bar[1]);
     }
+    __syncthreads();
     mbar_wait(&bar[0], 0);
+    mbar_wait(&bar[2], 0);
 
     CTile<UR, UC> ut{us, j0 - 2};
 #pragma unroll

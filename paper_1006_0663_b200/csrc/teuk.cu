@@ -80,7 +80,7 @@ struct teuk_ctx {
     cudaStream_t stream;
     SetupConsts C;
     // options
-    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0, theta_order = 2;
+    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0, theta_order = 2, opt_pdl = 0;   // PDL measured neutral on cfg 2 (40.2 vs 40.0 us): kept as an option
     ThetaWeights tw;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
     bool use_tma = false, use_rc = false, use_col_tma = false;
@@ -354,6 +354,8 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     } else if (!strcmp(key, "tile_j")) {
         if (v < 0 || v > 256) return TEUK_EINVAL;
         c->opt_tj = v;
+    } else if (!strcmp(key, "pdl")) {
+        c->opt_pdl = v != 0;
     } else if (!strcmp(key, "theta_order")) {
         if ((v != 2 && v != 10) || c->n_theta < v / 2) return TEUK_EINVAL;
         c->theta_order = v;
@@ -604,13 +606,25 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         int threads = 256;
         const void* fn = col_fn(c, &threads);
         if (cudaLaunchKernel(fn, c->grid, dim3(threads), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
-    } else if (c->use_rc) {
-        RcParams Q{c->dptr(c->lay.rc_th)};
-        if (c->tj == 8) step_kernel_f64_rc<32, 8><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);
-        else step_kernel_f64_rc<32, 16><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);
-    } else if (c->use_tma) {
-        if (c->tj == 8) step_kernel_f64_tma<32, 8><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ch, c->tm_ci, P);
-        else step_kernel_f64_tma<32, 16><<<c->grid, 256, c->smem, c->stream>>>(c->tm_state[from], c->tm_ch, c->tm_ci, P);
+    } else if (c->use_rc || c->use_tma) {
+        // programmatic dependent launch: the next step's blocks may start (and prefetch their coefficient tiles) while this
+        // step drains; they execute griddepcontrol.wait before touching the state
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = c->grid; cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = c->smem; cfg.stream = c->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = c->opt_pdl ? 1 : 0;
+        cudaError_t le;
+        if (c->use_rc) {
+            RcParams Q{c->dptr(c->lay.rc_th)};
+            if (c->tj == 8) le = cudaLaunchKernelEx(&cfg, step_kernel_f64_rc<32, 8>, c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);
+            else le = cudaLaunchKernelEx(&cfg, step_kernel_f64_rc<32, 16>, c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);
+        } else {
+            if (c->tj == 8) le = cudaLaunchKernelEx(&cfg, step_kernel_f64_tma<32, 8>, c->tm_state[from], c->tm_ch, c->tm_ci, P);
+            else le = cudaLaunchKernelEx(&cfg, step_kernel_f64_tma<32, 16>, c->tm_state[from], c->tm_ch, c->tm_ci, P);
+        }
+        if (le != cudaSuccess) return cuda_fail(le, "cudaLaunchKernelEx(step kernel)", __LINE__);
     } else {
         void* args[] = {&P};
         int threads = 256;
