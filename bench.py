@@ -232,13 +232,13 @@ def load_traffic(name):
 def run_sweep(args):
     """BASELINE.json config 5 (a = 0.99, s = -2, m = 2): updates/s and roofline fraction per cell.  fp64: HBM fraction
     (192 B/update vs MEASURED_PEAKS hbm_gbs); dd/qd: FP64-pipe fraction = measured FP64 thread instructions per update
-    (ncu, profiles/r01b_step_kernels_ncu.md: 1345 dd, 13630 qd FP64 instructions per update, redundant halo work included) x updates/s / measured DFMA-chain peak."""
+    (ncu, profiles/r01b_step_kernels_ncu.md: 1294 dd, 13320 qd FP64 instructions per update (profiles/r01c_dd_qd_ncu.md), redundant halo work included) x updates/s / measured DFMA-chain peak."""
     import torch
     from paper_1006_0663_b200 import teuk
     torch.cuda.set_device(0)
     peak, _ = measured_peaks()
     pipe = teuk.bench_fp64("dadd")
-    inst = {2: 1345.0, 4: 13630.0}
+    inst = {2: 1294.0, 4: 13320.0}
     for L in (1, 2, 4):
         for nr in (4096, 16384, 65536):
             for nt in (32, 64, 256):

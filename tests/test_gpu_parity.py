@@ -401,6 +401,35 @@ def test_full_size_configs_windowed(teuk, cfg, steps_gpu, k):
     print(cfg, worst)
 
 
+@pytest.mark.parametrize("n_r,n_t,L", [(4096, 32, 1), (4096, 256, 1), (16384, 64, 2), (4096, 256, 2), (4096, 64, 4), (65536, 32, 1)])
+def test_sweep_cells_prefix_windowed(teuk, n_r, n_t, L):
+    """BASELINE.json config 5 (a = 0.99, s = -2, m = 2) cells in the launch geometry bench.py --sweep times: 60-step GPU
+    prefix, then k more steps checked against oracle windows (inner wall, pulse, outer wall)"""
+    w = inputs.sweep_cell(n_r, n_t, L)
+    u0 = inputs.initial_state(w)
+    pre, k = 60, 6
+    g = run_gpu(teuk, w, u0, pre)
+    mid = g.read()
+    assert np.isfinite(mid).all()
+    g.step(k)
+    fin = g.read()
+    i_c = int((inputs.pulse_parameters(w)[0] - w.rstar_min) / w.dr)
+    n_win = 40
+    for i_lo in (0, i_c - n_win // 2, n_r - n_win):
+        o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win)
+        o.set_initial(np.ascontiguousarray(mid[..., i_lo:i_lo + n_win]))
+        o.step(k)
+        ref = o.read()
+        a, b = (0 if i_lo == 0 else k + 1), (n_win if i_lo + n_win == n_r else n_win - k - 1)
+        got = np.ascontiguousarray(fin[..., i_lo:i_lo + n_win][..., a:b])
+        want = np.ascontiguousarray(ref[..., a:b])
+        for re, im in ((0, 1), (2, 3)):
+            dre, _ = oracle._limb_diff(got[re], want[re])
+            dim, _ = oracle._limb_diff(got[im], want[im])
+            den = np.hypot(fin[re, 0], fin[im, 0]).max()
+            assert float(np.hypot(dre, dim).max() / den) <= TOL[L], (n_r, n_t, L, i_lo, re)
+
+
 def test_config2_prefix_full_grid_fp64(teuk):
     """config 2 at full size against the full-grid oracle for a 1000-step prefix (observer included)."""
     w = inputs.config(2)
