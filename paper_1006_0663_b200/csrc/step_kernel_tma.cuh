@@ -240,6 +240,7 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
     constexpr int UC = G::UC, UR = G::UR, HC = G::HC, HR = G::HR, CC = G::CC, NT = G::NT;
     extern __shared__ __align__(128) unsigned char raw[];
     __shared__ __align__(8) uint64_t bar[3];
+    __shared__ double tht[4][TJ + 2];           // cj, sin^2, cos, Tth for rows j0-1 .. j0+TJ (shared-memory, not L1, latency)
     unsigned char* base = (unsigned char*)(((uintptr_t)raw + 127) & ~(uintptr_t)127);
     double* us = (double*)base;
     double* ish = (double*)(base + G::US_B);
@@ -261,6 +262,11 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
         mbar_expect_tx(&bar[2], HR * CC * 8 + NT * CC * 8);
         tma_load_3d(ish, &tm_ish, i0 - 2, j0 - 1, 0, &bar[2]);
         tma_load_3d(rth, &tm_rth, i0 - 2, 0, 0, &bar[2]);
+    }
+    if (tid < 4 * (TJ + 2)) {
+        int t = tid / (TJ + 2), r = tid - t * (TJ + 2);
+        int j = min(max(j0 - 1 + r, 0), P.n_theta - 1);
+        tht[t][r] = (t == 0) ? __ldg(P.cj + j) : __ldg(Q.th + (t - 1) * P.n_theta + j);
     }
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (tid == 0) {
@@ -287,10 +293,9 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
                 if (rm < 0) { rm = 0; sm = P.sigma; }
                 if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
                 R1 cjv;
-                cjv.x[0] = __ldg(P.cj + jh);
+                cjv.x[0] = tht[0][tr];
                 RcCoef cf;
-                rc_eval(cf, ish[tr * CC + tc + 1], rth + tc + 1, CC, __ldg(Q.th + jh), __ldg(Q.th + nt + jh),
-                        __ldg(Q.th + 2 * nt + jh));
+                rc_eval(cf, ish[tr * CC + tc + 1], rth + tc + 1, CC, tht[1][tr], tht[2][tr], tht[3][tr]);
                 R1 out[4];
                 substep<1>(ut, jh, rm, rp, sm, sp, tc + 1, tc + 2, cf, cjv, P.tq_half, true, out, out);
 #pragma unroll
@@ -323,9 +328,9 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
 #pragma unroll
             for (int c = 0; c < 4; ++c) bs[c] = ut.get(c, j, tc + 2);
             R1 cjv;
-            cjv.x[0] = __ldg(P.cj + j);
+            cjv.x[0] = tht[0][tr + 1];
             RcCoef cf;
-            rc_eval(cf, isi[tr * TI + tc], rti + tc, TI, __ldg(Q.th + j), __ldg(Q.th + nt + j), __ldg(Q.th + 2 * nt + j));
+            rc_eval(cf, isi[tr * TI + tc], rti + tc, TI, tht[1][tr + 1], tht[2][tr + 1], tht[3][tr + 1]);
             substep<1>(ht, j, rm, rp, sm, sp, tc, tc + 1, cf, cjv, P.tq_full, false, bs, out);
         }
         long g = (long)j * P.pitch + i;

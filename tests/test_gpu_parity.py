@@ -464,6 +464,34 @@ def test_config2_full_length_fp64(teuk):
         assert max(res[cv][1].values()) <= TOL[1], cv
 
 
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_full_length_precision_ladder_on_gpu(teuk, cfg):
+    """BASELINE.json configs 3 and 4 at FULL size and FULL length (20000 / 50000 steps), which the oracle cannot reach
+    in test time: the same run at the three precisions must form a ladder (a property that holds at any size) —
+    fp64 agrees with dd to fp64 accuracy, dd with qd to dd accuracy — and stay finite.  Observer series included."""
+    w = inputs.config(cfg)
+    u0 = inputs.initial_state(w)
+    out = {}
+    for L in (1, 2, 4):
+        g = run_gpu(teuk, w, u0, w.steps, precision=L, observer=w.observer)
+        u, ser = g.read(), g.observe(w.steps)
+        assert np.isfinite(u).all() and ser.shape[0] == w.steps
+        pad = np.zeros((4, 4) + u.shape[2:])
+        pad[:, :L] = u
+        sp = np.zeros((w.steps, 4, 4))
+        sp[:, :, :L] = ser
+        out[L] = (pad, sp)
+        g.close()
+    e12 = oracle.rel_linf(out[1][0], out[2][0])
+    e24 = oracle.rel_linf(out[2][0], out[4][0])
+    s12 = series_err(out[1][1], out[2][1])
+    s24 = series_err(out[2][1], out[4][1])
+    print("cfg", cfg, "full length ladder: fp64-dd", e12, s12, "dd-qd", e24, s24)
+    assert max(e12.values()) <= 1e-11 and max(s12.values()) <= 1e-11
+    assert max(e24.values()) <= 1e-26 and max(s24.values()) <= 1e-26
+    assert max(e24.values()) > 0 and max(e12.values()) > 1e-18          # the rungs are distinct
+
+
 # ------------------------------------------------------------------------------- invariants and edge cases
 @pytest.mark.parametrize("L", [1, 2, 4])
 def test_gpu_exact_invariants(teuk, L):
