@@ -78,7 +78,8 @@ int teuk_observe(teuk_ctx *, double *host_out, long max_samples, long *count);
  * a_l' = integral of Phi(r*_obs, theta) _sY_l'm(theta) over the sphere, l' = l_min .. l_min + n_ell - 1 with
  * l_min = max(|s|, |m|), 1 <= n_ell <= 9, Fejer's first quadrature rule on the cell-centred theta grid (exact for
  * polynomials of degree < n_theta in cos(theta)), linear interpolation in r*.
- * capacity <= obs_capacity of teuk_create.  Call before teuk_set_initial or between teuk_step calls. */
+ * capacity <= obs_capacity of teuk_create.  Call before teuk_set_initial or between teuk_step calls; the sample index is
+ * shared with the point observer (both series restart at teuk_set_observer / teuk_set_initial). */
 int teuk_set_multipole_observer(teuk_ctx *, double rstar_obs, int n_ell, long capacity);
 /* host_out[count][n_ell][2][L]: real and imaginary part of a_l' per completed iteration; synchronises. */
 int teuk_observe_multipoles(teuk_ctx *, double *host_out, long max_samples, long *count);

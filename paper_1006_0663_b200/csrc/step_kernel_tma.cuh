@@ -85,7 +85,8 @@ __global__ void __launch_bounds__(256) step_kernel_f64_tma(const __grid_constant
     constexpr int UC = G::UC, UR = G::UR, HC = G::HC, HR = G::HR, CC = G::CC;
     extern __shared__ __align__(128) unsigned char raw[];
     __shared__ __align__(8) uint64_t bar[3];
-    unsigned char* base = (unsigned char*)(((uintptr_t)raw + 127) & ~(uintptr_t)127);
+    unsigned char* base = raw;      // __align__(128) on the extern array is honoured; no integer round trip, so the
+                                    // compiler keeps these pointers in the shared state space (LDS/STS, not generic LD/ST)
     double* us = (double*)base;
     double* chs = (double*)(base + G::US_B);
     double* cis = (double*)(base + G::US_B + G::CH_B);
@@ -241,7 +242,8 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
     extern __shared__ __align__(128) unsigned char raw[];
     __shared__ __align__(8) uint64_t bar[3];
     __shared__ double tht[4][TJ + 2];           // cj, sin^2, cos, Tth for rows j0-1 .. j0+TJ (shared-memory, not L1, latency)
-    unsigned char* base = (unsigned char*)(((uintptr_t)raw + 127) & ~(uintptr_t)127);
+    unsigned char* base = raw;      // __align__(128) on the extern array is honoured; no integer round trip, so the
+                                    // compiler keeps these pointers in the shared state space (LDS/STS, not generic LD/ST)
     double* us = (double*)base;
     double* ish = (double*)(base + G::US_B);
     double* isi = (double*)(base + G::US_B + G::ISH_B);
@@ -386,7 +388,8 @@ __global__ void __launch_bounds__(256) step_kernel_f64_col_tma(const __grid_cons
     __shared__ __align__(8) uint64_t bar[2];
     const int nt = P.n_theta, nr = P.n_r;
     auto a128 = [](size_t v) { return (v + 127) / 128 * 128; };
-    unsigned char* base = (unsigned char*)(((uintptr_t)raw + 127) & ~(uintptr_t)127);
+    unsigned char* base = raw;      // __align__(128) on the extern array is honoured; no integer round trip, so the
+                                    // compiler keeps these pointers in the shared state space (LDS/STS, not generic LD/ST)
     double* us = (double*)base;                      base += a128((size_t)4 * nt * UC * 8);
     double* ish = (double*)base;                     base += a128((size_t)nt * CC * 8);
     double* isi = (double*)base;                     base += a128((size_t)nt * TI * 8);

@@ -93,6 +93,7 @@ struct teuk_ctx {
     bool have_init = false;
     int cur = 0;                       // which state buffer holds u^n
     long steps_done = 0, launches = 0;
+    long series_origin = 0;            // steps_done when the sample counter was last reset (set_observer / set_initial)
     // observer
     long obs_cap = 0;
     int oi = 0, oj = 0;
@@ -389,6 +390,7 @@ extern "C" int teuk_set_observer(teuk_ctx* c, double rstar_obs, double theta_obs
     for (int p = 0; p < 2; ++p)
         if (c->graph[p]) { cudaGraphExecDestroy(c->graph[p]); c->graph[p] = nullptr; }
     CK(cudaMemsetAsync(c->step_base(), 0, 32, c->stream));
+    c->series_origin = c->steps_done;      // both series (point observer and multipoles) restart here
     return TEUK_OK;
 }
 
@@ -651,7 +653,7 @@ static int upload_initial(teuk_ctx* c, const double* d_src, int limbs_in) {
     c->launches++;
     if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
     CK(cudaMemsetAsync(c->step_base(), 0, 32, c->stream));
-    c->cur = 0; c->steps_done = 0; c->nonfinite = false;
+    c->cur = 0; c->steps_done = 0; c->series_origin = 0; c->nonfinite = false;
     if (!c->have_init) {
         int rc = choose_geometry(c);
         if (rc != TEUK_OK) return rc;
@@ -746,7 +748,8 @@ extern "C" int teuk_read(teuk_ctx* c, double* host_planes) {
 
 extern "C" int teuk_observe(teuk_ctx* c, double* host_out, long max_samples, long* count) {
     if (!c || !host_out || !count || max_samples < 0) return TEUK_EINVAL;
-    long n = c->steps_done < c->obs_cap ? c->steps_done : c->obs_cap;
+    long n = c->steps_done - c->series_origin;
+    if (n > c->obs_cap) n = c->obs_cap;
     if (n > max_samples) n = max_samples;
     if (n > 0) {
         unsigned blocks = (unsigned)((n * 4 + 127) / 128);
@@ -858,7 +861,8 @@ extern "C" int teuk_set_multipole_observer(teuk_ctx* c, double rstar_obs, int n_
 
 extern "C" int teuk_observe_multipoles(teuk_ctx* c, double* host_out, long max_samples, long* count) {
     if (!c || !host_out || !count || max_samples < 0) return TEUK_EINVAL;
-    long n = c->steps_done < c->mp_cap ? c->steps_done : c->mp_cap;
+    long n = c->steps_done - c->series_origin;
+    if (n > c->mp_cap) n = c->mp_cap;
     if (n > max_samples) n = max_samples;
     if (n > 0)
         CK(cudaMemcpyAsync(host_out, c->dptr(c->lay.mp_series), (size_t)n * c->mp_n * 2 * c->L * sizeof(double),

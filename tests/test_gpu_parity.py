@@ -512,6 +512,26 @@ def test_gpu_exact_invariants(teuk, L):
     assert np.array_equal(g4.read(), u)
 
 
+def test_observer_reset_mid_run(teuk):
+    """teuk_set_observer between teuk_step calls restarts the series at the current step"""
+    w = inputs.config(1).scaled(n_r=96)
+    u0 = inputs.initial_state(w)
+    g = teuk.Teuk.from_workload(w, obs_capacity=50)
+    g.set_observer(40.0, 1.2, 50)
+    g.set_initial(u0)
+    g.step(20)
+    assert g.observe(50).shape[0] == 20
+    g.set_observer(30.0, 1.0, 50)
+    assert g.observe(50).shape[0] == 0
+    g.step(7)
+    got = g.observe(50)
+    assert got.shape[0] == 7
+    o = run_oracle(w, u0, 20)
+    o.set_observer(30.0, 1.0, 50)
+    o.step(7)
+    assert max(series_err(got, o.observe(50)).values()) <= TOL[1]
+
+
 def test_edge_cases_and_errors(teuk):
     import ctypes
     # smallest legal grid, odd m, zero steps
