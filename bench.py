@@ -340,6 +340,12 @@ def main():
             ach = 80.0 * points / (msr / args.steps * 1e-3) / 1e9
             line["semi_recompute"] = {"updates_per_s": points * args.steps / (msr * 1e-3), "ms_per_step": msr / args.steps,
                                       "algorithmic_bytes_per_update": 80.0, "hbm_frac": ach / peak, "geometry": gr, "finite": fr}
+            # NEXT-3: two iterations per launch (u^{n+1} and the coefficient tiles stay on the SM): 96 B/update
+            mst, lt, gt, ft = time_device(torch, teuk, w, args.steps, args.warmup, list(args.option) + ["time_block=2"])
+            acht = 96.0 * points / (mst / args.steps * 1e-3) / 1e9
+            line["time_blocked_2"] = {"updates_per_s": points * args.steps / (mst * 1e-3), "ms_per_step": mst / args.steps,
+                                      "algorithmic_bytes_per_update": 96.0, "hbm_frac": acht / peak, "gpu_launches": lt,
+                                      "geometry": gt, "finite": ft}
         line["per_precision"] = per
         line["fp64_pipe_peak_inst_per_s"] = fp
         line["cpu_baseline"] = cpu_baseline(w)

@@ -1,0 +1,26 @@
+// Instantiations of the fp64 TMA step kernels (step_kernel_tma.cuh).
+#include "kernels.h"
+#include "step_kernel_tma.cuh"
+
+namespace tk {
+
+const void* tma_step_fn(int ti, int tj) {
+    if (ti != 32) return nullptr;
+    if (tj == 8) return (const void*)step_kernel_f64_tma<32, 8>;
+    if (tj == 16) return (const void*)step_kernel_f64_tma<32, 16>;
+    return nullptr;
+}
+const void* rc_step_fn(int ti, int tj) {
+    if (ti != 32) return nullptr;
+    if (tj == 8) return (const void*)step_kernel_f64_rc<32, 8>;
+    if (tj == 16) return (const void*)step_kernel_f64_rc<32, 16>;
+    return nullptr;
+}
+const void* col_tma_fn(int ti) {
+    if (ti == 8) return (const void*)step_kernel_f64_col_tma<8>;
+    if (ti == 12) return (const void*)step_kernel_f64_col_tma<12>;
+    if (ti == 16) return (const void*)step_kernel_f64_col_tma<16>;
+    return nullptr;
+}
+
+}  // namespace tk

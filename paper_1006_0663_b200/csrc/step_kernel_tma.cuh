@@ -483,14 +483,4 @@ __global__ void __launch_bounds__(256) step_kernel_f64_col_tma(const __grid_cons
     }
 }
 
-// test hook: recomputed folded coefficients of one family written as 8 planes [n_theta][pitch]
-__global__ void rc_tables_kernel(const double* __restrict__ isig, const double* __restrict__ rt, const double* __restrict__ th,
-                                 int cols, int n_theta, int pitch, long plane, double* __restrict__ out) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
-    if (i >= cols) return;
-    RcCoef cf;
-    rc_eval(cf, isig[(long)j * pitch + i], rt + i, pitch, th[j], th[n_theta + j], th[2 * n_theta + j]);
-    for (int q = 0; q < 8; ++q) out[q * plane + (long)j * pitch + i] = cf.c[q];
-}
-
 }  // namespace tk

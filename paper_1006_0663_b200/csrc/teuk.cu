@@ -16,6 +16,8 @@
 #include "setup_math.cuh"
 #include "step_kernel.cuh"
 #include "step_kernel_tma.cuh"
+#include "step_kernel_tb2.cuh"
+#include "kernels.h"
 
 using namespace tk;
 
@@ -80,11 +82,16 @@ struct teuk_ctx {
     cudaStream_t stream;
     SetupConsts C;
     // options
-    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0, theta_order = 2, opt_pdl = 0;   // PDL measured neutral on cfg 2 (40.2 vs 40.0 us): kept as an option
+    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0, theta_order = 2, opt_pdl = 0, opt_tb = 1;   // PDL measured neutral on cfg 2 (40.2 vs 40.0 us): kept as an option
     ThetaWeights tw;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
     bool use_tma = false, use_rc = false, use_col_tma = false;
     CUtensorMap tm_state[2], tm_ch, tm_ci, tm_ish, tm_isi, tm_rth, tm_rti;
+    // temporally blocked fp64 path (two iterations per launch, step_kernel_tb2.cuh): its own boxes, grid and smem
+    bool use_tb2 = false;
+    CUtensorMap tm2_state[2], tm2_ch;
+    dim3 grid2;
+    size_t smem2 = 0;
     // geometry
     int ti = 0, tj = 0, threads = 256;
     dim3 grid;
@@ -366,6 +373,9 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     } else if (!strcmp(key, "variant")) {
         if (v < 0 || v > 2) return TEUK_EINVAL;
         c->variant = v;
+    } else if (!strcmp(key, "time_block")) {
+        if ((v != 1 && v != 2) || (v == 2 && c->L != 1)) return TEUK_EINVAL;
+        c->opt_tb = v;
     } else if (!strcmp(key, "use_tma")) {
         c->opt_tma = v != 0;
     } else {
@@ -429,30 +439,32 @@ template <int TI, int TJ> static bool setup_tma(teuk_ctx* c) {
               make_map(&c->tm_ch, c->dptr(y.coef_h), c->n_r - 1, c->n_theta, 8, y.pitch, y.plane, G::CC, G::HR, 8) &&
               make_map(&c->tm_ci, c->dptr(y.coef_i), c->n_r, c->n_theta, 8, y.pitch, y.plane, TI, TJ, 8);
     if (!ok) return false;
-    if (cudaFuncSetAttribute(step_kernel_f64_tma<TI, TJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::TOTAL) != cudaSuccess)
-        return false;
+    const void* fn = tma_step_fn(TI, TJ);
+    if (!fn || cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, G::TOTAL) != cudaSuccess) return false;
     c->ti = TI; c->tj = TJ; c->smem = G::TOTAL; c->threads = 256;
     c->grid = dim3((c->n_r + TI - 1) / TI, (c->n_theta + TJ - 1) / TJ);
     return true;
 }
 
-// instantiation table of the generic kernel: (precision, variant, tile) -> function and block size
+template <int TI, int TJ> static bool setup_tb2(teuk_ctx* c) {
+    using G = Tb2Geom<TI, TJ>;
+    const Layout& y = c->lay;
+    bool ok = make_map(&c->tm2_state[0], c->state(0), c->n_r, c->n_theta, 4, y.pitch, y.plane, G::UC, G::UR, 4) &&
+              make_map(&c->tm2_state[1], c->state(1), c->n_r, c->n_theta, 4, y.pitch, y.plane, G::UC, G::UR, 4) &&
+              make_map(&c->tm2_ch, c->dptr(y.coef_h), c->n_r - 1, c->n_theta, 8, y.pitch, y.plane, G::CC, G::H1R, 8);
+    if (!ok) return false;
+    const void* fn = tb2_step_fn(TI, TJ);
+    if (!fn || cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, G::TOTAL) != cudaSuccess) return false;
+    c->smem2 = G::TOTAL;
+    c->grid2 = dim3((c->n_theta + TJ - 1) / TJ, (c->n_r + TI - 1) / TI);      // theta tiles fastest
+    return c->grid2.y <= 65535;
+}
+
+// instantiation tables of the generic kernels live in k_generic{1,2,4}.cu: (precision, variant, tile) -> function, block size
 static const void* step_fn(const teuk_ctx* c, int* threads) {
-    *threads = 256;
-    if (c->L == 1) return (const void*)step_kernel<1, 0, 0, 256, 4>;
-    if (c->L == 2) {
-        if (c->variant == 1) { *threads = 128; return (const void*)step_kernel<2, 0, 0, 128, 5>; }
-        if (c->variant == 2) { *threads = 128; return (const void*)step_kernel<2, 0, 0, 128, 6>; }
-        if (c->ti == 32 && c->tj == 16) return (const void*)step_kernel<2, 32, 16, 256, 2>;
-        if (c->ti == 64 && c->tj == 8) return (const void*)step_kernel<2, 64, 8, 256, 2>;
-        return (const void*)step_kernel<2, 0, 0, 256, 2>;
-    }
-    // qd: 128 threads x 3 blocks/SM (168 registers, a few spills) measured 1.9x faster than 256 x 1 (254 registers)
-    if (c->variant == 1) return (const void*)step_kernel<4, 0, 0, 256, 1>;
-    *threads = 128;
-    if (c->variant == 2) return (const void*)step_kernel<4, 0, 0, 128, 4>;
-    if (c->ti == 16 && c->tj == 8) return (const void*)step_kernel<4, 16, 8, 128, 3>;
-    return (const void*)step_kernel<4, 0, 0, 128, 3>;
+    if (c->L == 1) return generic_step_fn_1(c->variant, c->ti, c->tj, threads);
+    if (c->L == 2) return generic_step_fn_2(c->variant, c->ti, c->tj, threads);
+    return generic_step_fn_4(c->variant, c->ti, c->tj, threads);
 }
 
 template <int TI, int TJ> static bool setup_rc(teuk_ctx* c) {
@@ -467,8 +479,8 @@ template <int TI, int TJ> static bool setup_rc(teuk_ctx* c) {
               make_map(&c->tm_rti, rt0, c->n_r, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, TI, RC_NT, 1) &&
               make_map(&c->tm_rth, rt0 + (size_t)RC_NT * y.pitch, c->n_r - 1, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, G::CC, RC_NT, 1);
     if (!ok) return false;
-    if (cudaFuncSetAttribute(step_kernel_f64_rc<TI, TJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::TOTAL) != cudaSuccess)
-        return false;
+    const void* fn = rc_step_fn(TI, TJ);
+    if (!fn || cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, G::TOTAL) != cudaSuccess) return false;
     c->ti = TI; c->tj = TJ; c->smem = G::TOTAL; c->threads = 256;
     c->grid = dim3((c->n_r + TI - 1) / TI, (c->n_theta + TJ - 1) / TJ);
     return true;
@@ -488,19 +500,17 @@ template <int TI> static bool setup_col_tma(teuk_ctx* c) {
               make_map(&c->tm_rth, rt0 + (size_t)RC_NT * y.pitch, c->n_r - 1, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, G::CC, RC_NT, 1);
     size_t sm = G::total(nt);
     if (!ok || sm > 227 * 1024) return false;
-    if (cudaFuncSetAttribute(step_kernel_f64_col_tma<TI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
-        return false;
+    const void* fn = col_tma_fn(TI);
+    if (!fn || cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess) return false;
     c->ti = TI; c->tj = nt; c->smem = sm; c->threads = 256;
     c->grid = dim3((c->n_r + TI - 1) / TI, 1);
     return true;
 }
 
 static const void* col_fn(const teuk_ctx* c, int* threads) {
-    *threads = 256;
-    if (c->L == 1) return (const void*)step_kernel_col<1, 256, 2>;
-    if (c->L == 2) return (const void*)step_kernel_col<2, 256, 2>;
-    *threads = 128;
-    return (const void*)step_kernel_col<4, 128, 3>;
+    if (c->L == 1) return generic_col_fn_1(threads);
+    if (c->L == 2) return generic_col_fn_2(threads);
+    return generic_col_fn_4(threads);
 }
 
 // centred 11-point weights from the textbook closed form c_k = (-1)^(k+1) (N!)^2 / (k (N-k)! (N+k)!), d_k = 2 c_k / k
@@ -522,6 +532,8 @@ static void fill_theta_weights(ThetaWeights& w) {
 static int choose_geometry(teuk_ctx* c) {
     c->use_tma = false;
     c->use_rc = false;
+    c->use_tb2 = false;
+    if (c->opt_tb == 2 && (c->theta_order == 10 || c->coef_variant != 0)) return TEUK_EINVAL;
     if (c->theta_order == 10) {
         fill_theta_weights(c->tw);
         c->use_col_tma = false;
@@ -559,8 +571,19 @@ static int choose_geometry(teuk_ctx* c) {
     if (c->L == 1 && c->opt_tma && (c->opt_ti == 0 || c->opt_ti == 32) && (c->opt_tj == 0 || c->opt_tj == 8 || c->opt_tj == 16)) {
         bool ok = (c->opt_tj == 8) ? setup_tma<32, 8>(c) : setup_tma<32, 16>(c);
         cudaGetLastError();
-        if (ok) { c->use_tma = true; return TEUK_OK; }
+        if (ok) {
+            c->use_tma = true;
+            if (c->opt_tb == 2) {
+                // two iterations per launch on the same output tile; the single-step kernel serves an odd last step
+                bool ok2 = (c->tj == 8) ? setup_tb2<32, 8>(c) : setup_tb2<32, 16>(c);
+                cudaGetLastError();
+                if (!ok2) return TEUK_ECUDA;
+                c->use_tb2 = true;
+            }
+            return TEUK_OK;
+        }
     }
+    if (c->opt_tb == 2) return TEUK_EINVAL;        // time blocking exists only on the fp64 TMA stored-plane path
     int ti = c->opt_ti, tj = c->opt_tj;
     if (ti == 0) ti = (c->L == 4) ? 16 : 32;
     if (tj == 0) {
@@ -599,10 +622,8 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
     P.oi = c->oi; P.oj = c->oj;
     if (c->theta_order == 10 && c->use_col_tma) {
         RcParams Q{c->dptr(c->lay.rc_th)};
-        const CUtensorMap& tu = c->tm_state[from];
-        if (c->ti == 16) step_kernel_f64_col_tma<16><<<c->grid, 256, c->smem, c->stream>>>(tu, c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q, c->tw);
-        else if (c->ti == 12) step_kernel_f64_col_tma<12><<<c->grid, 256, c->smem, c->stream>>>(tu, c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q, c->tw);
-        else step_kernel_f64_col_tma<8><<<c->grid, 256, c->smem, c->stream>>>(tu, c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q, c->tw);
+        void* args[] = {&c->tm_state[from], &c->tm_ish, &c->tm_isi, &c->tm_rth, &c->tm_rti, &P, &Q, &c->tw};
+        if (cudaLaunchKernel(col_tma_fn(c->ti), c->grid, dim3(256), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
     } else if (c->theta_order == 10) {
         void* args[] = {&P, &c->tw};
         int threads = 256;
@@ -618,13 +639,13 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at; cfg.numAttrs = c->opt_pdl ? 1 : 0;
         cudaError_t le;
+        RcParams Q{c->dptr(c->lay.rc_th)};
         if (c->use_rc) {
-            RcParams Q{c->dptr(c->lay.rc_th)};
-            if (c->tj == 8) le = cudaLaunchKernelEx(&cfg, step_kernel_f64_rc<32, 8>, c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);
-            else le = cudaLaunchKernelEx(&cfg, step_kernel_f64_rc<32, 16>, c->tm_state[from], c->tm_ish, c->tm_isi, c->tm_rth, c->tm_rti, P, Q);
+            void* args[] = {&c->tm_state[from], &c->tm_ish, &c->tm_isi, &c->tm_rth, &c->tm_rti, &P, &Q};
+            le = cudaLaunchKernelExC(&cfg, rc_step_fn(c->ti, c->tj), args);
         } else {
-            if (c->tj == 8) le = cudaLaunchKernelEx(&cfg, step_kernel_f64_tma<32, 8>, c->tm_state[from], c->tm_ch, c->tm_ci, P);
-            else le = cudaLaunchKernelEx(&cfg, step_kernel_f64_tma<32, 16>, c->tm_state[from], c->tm_ch, c->tm_ci, P);
+            void* args[] = {&c->tm_state[from], &c->tm_ch, &c->tm_ci, &P};
+            le = cudaLaunchKernelExC(&cfg, tma_step_fn(c->ti, c->tj), args);
         }
         if (le != cudaSuccess) return cuda_fail(le, "cudaLaunchKernelEx(step kernel)", __LINE__);
     } else {
@@ -644,6 +665,38 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         else multipole_kernel<4><<<1, threads, sm, c->stream>>>(uo, qd_, ser, c->step_base(), step_off, c->mp_cap, c->mp_n, c->n_theta, c->lay.pitch, c->lay.plane, c->mp_i, c->mp_wr);
     }
     return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+}
+
+static inline bool tb2_active(const teuk_ctx* c) { return c->use_tb2 && c->mp_cap == 0; }
+
+// two iterations in one launch: state(from) = u^n  ->  state(from ^ 1) = u^{n+2}; observer samples step_off, step_off + 1
+static int launch_step2(teuk_ctx* c, int from, int step_off) {
+    StepParams P;
+    P.u_in = c->state(from);
+    P.u_out = c->state(from ^ 1);
+    P.coef_i = c->dptr(c->lay.coef_i);
+    P.coef_h = c->dptr(c->lay.coef_h);
+    P.cj = c->dptr(c->lay.cj);
+    P.n_r = c->n_r; P.n_theta = c->n_theta; P.pitch = c->lay.pitch; P.plane = c->lay.plane;
+    P.ti = c->ti; P.tj = c->tj;
+    P.sigma = (std::abs(c->m) % 2 == 0) ? 1.0 : -1.0;
+    P.tq_half = 0.25 * c->dt;
+    P.tq_full = 0.5 * c->dt;
+    P.obs_raw = c->obs_cap > 0 ? c->dptr(c->lay.obs_raw) : nullptr;
+    P.step_base = c->step_base();
+    P.obs_cap = c->obs_cap;
+    P.step_off = step_off;
+    P.oi = c->oi; P.oj = c->oj;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = c->grid2; cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = c->smem2; cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = c->opt_pdl ? 1 : 0;
+    void* args[] = {&c->tm2_state[from], &c->tm2_ch, &P};
+    cudaError_t le = cudaLaunchKernelExC(&cfg, tb2_step_fn(c->ti, c->tj), args);
+    if (le != cudaSuccess) return cuda_fail(le, "cudaLaunchKernelExC(step2 kernel)", __LINE__);
+    return TEUK_OK;
 }
 
 static int upload_initial(teuk_ctx* c, const double* d_src, int limbs_in) {
@@ -682,8 +735,9 @@ static int build_graph(teuk_ctx* c, int parity) {
     cudaGraph_t g;
     CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
     int from = parity, rc = TEUK_OK;
-    for (int k = 0; k < c->graph_steps && rc == TEUK_OK; ++k) {
-        rc = launch_step(c, from, k);
+    const int stride = tb2_active(c) ? 2 : 1;       // graph_steps is even
+    for (int k = 0; k < c->graph_steps && rc == TEUK_OK; k += stride) {
+        rc = stride == 2 ? launch_step2(c, from, k) : launch_step(c, from, k);
         from ^= 1;
     }
     advance_kernel<<<1, 1, 0, c->stream>>>(c->step_base(), c->graph_steps);
@@ -706,17 +760,28 @@ extern "C" int teuk_step(teuk_ctx* c, long n) {
             if (rc != TEUK_OK) return rc;
         }
         CK(cudaGraphLaunch(c->graph[c->cur], c->stream));
-        c->launches += (c->mp_cap > 0 ? 2 * K : K) + 1;
-        left -= K;                            // K is even: c->cur unchanged
+        if (tb2_active(c)) {
+            c->launches += K / 2 + 1;
+            c->cur ^= (K / 2) & 1;            // one buffer flip per two-iteration launch
+        } else {
+            c->launches += (c->mp_cap > 0 ? 2 * K : K) + 1;      // K is even: c->cur unchanged
+        }
+        left -= K;
     }
     if (left > 0) {
-        for (long k = 0; k < left; ++k) {
+        long k = 0, nl = 0;
+        for (; tb2_active(c) && k + 2 <= left; k += 2, ++nl) {
+            int rc = launch_step2(c, c->cur, (int)k);
+            if (rc != TEUK_OK) return rc;
+            c->cur ^= 1;
+        }
+        for (; k < left; ++k, ++nl) {
             int rc = launch_step(c, c->cur, (int)k);
             if (rc != TEUK_OK) return rc;
             c->cur ^= 1;
         }
         advance_kernel<<<1, 1, 0, c->stream>>>(c->step_base(), left);
-        c->launches += (c->mp_cap > 0 ? 2 * left : left) + 1;
+        c->launches += (c->mp_cap > 0 ? 2 * nl : nl) + 1;
         if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
     }
     c->steps_done += n;
@@ -886,6 +951,7 @@ extern "C" int teuk_step_geometry(teuk_ctx* c, long* o) {
     if (!c || !o) return TEUK_EINVAL;
     if (!c->have_init) return TEUK_ESTATE;
     o[0] = c->ti; o[1] = c->tj; o[2] = c->threads; o[3] = c->grid.x; o[4] = c->grid.y; o[5] = (long)c->smem;
+    if (c->use_tb2) { o[3] = c->grid2.x; o[4] = c->grid2.y; o[5] = (long)c->smem2; }
     return TEUK_OK;
 }
 extern "C" void teuk_destroy(teuk_ctx* c) {
@@ -925,6 +991,16 @@ extern "C" int teuk_get_tables(teuk_ctx* c, int half, double* host_out) {
             for (int i = 0; i < rows; ++i)
                 host_out[((size_t)pl * c->n_theta + j) * rows + i] = h[(size_t)pl * c->lay.plane + (size_t)j * c->lay.pitch + i];
     return TEUK_OK;
+}
+
+// test hook: recomputed folded coefficients of one family written as 8 planes [n_theta][pitch]
+__global__ void rc_tables_kernel(const double* __restrict__ isig, const double* __restrict__ rt, const double* __restrict__ th,
+                                 int cols, int n_theta, int pitch, long plane, double* __restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= cols) return;
+    RcCoef cf;
+    rc_eval(cf, isig[(long)j * pitch + i], rt + i, pitch, th[j], th[n_theta + j], th[2 * n_theta + j]);
+    for (int q = 0; q < 8; ++q) out[q * plane + (long)j * pitch + i] = cf.c[q];
 }
 
 extern "C" int teuk_get_folded(teuk_ctx* c, int half, int coef_variant, double* host_out) {

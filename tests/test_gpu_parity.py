@@ -163,6 +163,81 @@ def test_tma_kernel_matches_generic_kernel_fp64(teuk, n_r, n_t):
     assert np.array_equal(outs["tma16"][0], outs["tma8"][0])
 
 
+# ------------------------------------------------------------------------------- NEXT-3: two iterations per launch (fp64)
+@pytest.mark.parametrize("n_r,n_t,steps", [(203, 13, 64), (512, 16, 65), (1000, 70, 37), (40, 3, 8), (33, 17, 21), (97, 64, 50)])
+@pytest.mark.parametrize("m,s", [(2, -2), (1, -1)])
+def test_time_blocked_kernel_fp64(teuk, n_r, n_t, steps, m, s):
+    """time_block=2 (step2_kernel_f64_tma: two iterations of Eqs. 13-14 per launch, u^{n+1} only in shared memory)
+    against the oracle and against the single-step kernel, on ragged grids, odd step counts (the last iteration falls to
+    the single-step kernel), both tile heights, even and odd |m| (ghost sign), with the observer sampled every step"""
+    w = inputs.config(2).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0, m=m, s=s)
+    w = w.scaled(dt_override=inputs.stable_dt(w))
+    u0 = inputs.random_state(n_r, n_t, 1, seed=33)
+    obs = (10.3, 1.1)
+    one = run_gpu(teuk, w, u0, steps, observer=obs)
+    outs = {}
+    for name, opts in (("tb16", {"time_block": 2}), ("tb8", {"time_block": 2, "tile_j": 8}),
+                       ("tb16_nograph", {"time_block": 2, "graph_steps": 0}), ("tb16_g2", {"time_block": 2, "graph_steps": 2})):
+        g = run_gpu(teuk, w, u0, steps, options=opts, observer=obs)
+        outs[name] = (g.read(), g.observe(steps))
+        assert g.steps_done() == steps
+    o = run_oracle(w, u0, steps, observer=obs)
+    ref, sref = o.read(), o.observe(steps)
+    for name, (u, ser) in outs.items():
+        assert ser.shape[0] == steps, name
+        assert max(oracle.rel_linf(u, ref).values()) <= TOL[1], name
+        assert max(series_err(ser, sref).values()) <= TOL[1], name
+        # same arithmetic as the single-step kernel (FMA contraction may differ between instantiations: a few ulps)
+        assert max(oracle.rel_linf(u, one.read()).values()) <= 1e-14, name
+    assert np.array_equal(outs["tb16"][0], outs["tb8"][0])
+    assert np.array_equal(outs["tb16"][0], outs["tb16_nograph"][0])
+    assert np.array_equal(outs["tb16"][0], outs["tb16_g2"][0])
+    assert np.array_equal(outs["tb16"][1], outs["tb16_g2"][1])
+
+
+def test_time_blocked_kernel_split_calls_and_invariants(teuk):
+    """teuk_step called in odd pieces equals one call; Dirichlet rows stay exactly zero; a = 0, s = m = 0 reflection
+    symmetry stays bit-exact; time_block=2 is refused where it does not exist (dd, theta_order 10, recompute supply)"""
+    w = inputs.config(1).scaled(n_r=600, n_theta=24)      # omega dt = 0.5: inside the stability bound (reading A15b)
+    u0 = inputs.initial_state(w)
+    a = run_gpu(teuk, w, u0, 101, options={"time_block": 2})
+    b = teuk.Teuk.from_workload(w)
+    b.set_option("time_block", 2)
+    b.set_initial(u0)
+    for n in (1, 2, 33, 64, 1):
+        b.step(n)
+    ua, ub = a.read(), b.read()
+    assert np.array_equal(ua, ub)
+    assert not ua[:, :, :, 0].any() and not ua[:, :, :, -1].any()
+    assert np.array_equal(ua, ua[:, :, ::-1, :])
+    o = run_oracle(w, u0, 101)
+    assert max(oracle.rel_linf(ua, o.read()).values()) <= TOL[1]
+    g = teuk.Teuk.from_workload(w, precision=2)
+    with pytest.raises(teuk.TeukError):
+        g.set_option("time_block", 2)
+    for bad in ({"theta_order": 10}, {"coef_variant": 1}, {"use_tma": 0}):
+        g = teuk.Teuk.from_workload(w)
+        g.set_option("time_block", 2)
+        for k, v in bad.items():
+            g.set_option(k, v)
+        with pytest.raises(teuk.TeukError):
+            g.set_initial(u0)
+
+
+def test_time_blocked_config2_prefix_full_grid(teuk):
+    """config 2 at full size in the bench launch geometry, time_block=2, 1000-step prefix vs the full-grid oracle"""
+    w = inputs.config(2)
+    u0 = inputs.initial_state(w)
+    steps = 1000
+    g = run_gpu(teuk, w, u0, steps, observer=w.observer, options={"time_block": 2})
+    o = run_oracle(w, u0, steps, observer=w.observer)
+    err = oracle.rel_linf(g.read(), o.read())
+    print("cfg2 prefix, time_block=2", err)
+    assert max(err.values()) <= TOL[1]
+    serr = series_err(g.observe(steps), o.observe(steps))
+    assert max(serr.values()) <= TOL[1] or np.abs(o.observe(steps)).max() < 1e-300
+
+
 # ------------------------------------------------------------------------------- semi-recompute coefficient supply (H1b)
 @pytest.mark.parametrize("cfg", [1, 2])
 def test_recomputed_coefficients_match_stored_planes(teuk, cfg):
