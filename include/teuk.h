@@ -39,13 +39,28 @@ int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double r
                 double dt, int precision, void *d_workspace, size_t workspace_bytes, long obs_capacity,
                 void *cuda_stream, teuk_ctx **out);
 
+/* Radial slab of the same problem (the paper's own domain decomposition):
+ * the handle holds columns i_lo .. i_lo + n_win - 1 of the uniform grid of n_r_global nodes on [rstar_min, rstar_max]
+ * (r*_i = rstar_min + (i_lo + i) dr*, dr* = (rstar_max - rstar_min)/(n_r_global - 1)): same tables, bit for bit, as the
+ * full-grid handle has at those columns.  State planes, teuk_read and the column calls use LOCAL indices 0 .. n_win-1;
+ * observer locations stay physical (r*, theta) and must fall inside the slab.  The slab's two edge columns are
+ * Dirichlet rows like any handle's: where an edge is a cut and not the physical boundary, the values
+ * within k columns of it are invalid k iterations after the caller last refreshed them (r* reach of Eqs. 13-14 is one
+ * column per iteration) - the caller keeps a halo and refreshes it with teuk_write_columns_device (see
+ * paper_1006_0663_b200/slabs.py).  0 <= i_lo, i_lo + n_win <= n_r_global, n_win >= 3; workspace sized for n_win. */
+int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_theta, double rstar_min, double rstar_max,
+                     double dt, int precision, int i_lo, int n_win, void *d_workspace, size_t workspace_bytes,
+                     long obs_capacity, void *cuda_stream, teuk_ctx **out);
+
 /* Options, only before teuk_set_initial (else TEUK_ESTATE): "graph_steps" (even, >= 2; steps per
  * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic), "use_tma" (fp64: 1 = TMA
  * kernel, default; 0 = generic kernel), "variant" (dd/qd launch shape 0..2), "coef_variant" (0 = precomputed
  * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only),
  * "pdl" (fp64 TMA kernels: 1 = programmatic dependent launch, the next step prefetches its half-step coefficient
  * tile while the current one drains; default 0, measured neutral), "theta_order" (2 = second-order centred theta differences, default; 10 = the 10th-order
- * 11-point operator of PAPER.md:126, needs n_theta >= 5). */
+ * 11-point operator of PAPER.md:126, needs n_theta >= 5), "time_block" (1 = one iteration per launch, default; 2 = two
+ * iterations per launch on a shared-memory resident tile, fp64 stored-plane TMA path only, else TEUK_EINVAL at
+ * teuk_set_initial; an odd last iteration and runs with the multipole observer use the one-iteration kernel). */
 int teuk_set_option(teuk_ctx *, const char *key, double value);
 
 /* Observer at a fixed location: bilinear interpolation in (r*, theta) from the four
@@ -68,6 +83,13 @@ int teuk_step(teuk_ctx *, long n);
 int teuk_read(teuk_ctx *, double *host_planes);
 /* Copy the state into DEVICE memory of the same layout; asynchronous on the stream. */
 int teuk_read_device(teuk_ctx *, double *d_planes);
+
+/* Column strips of the current state (halo exchange between slabs): d_out / d_in are DEVICE buffers
+ * double[4][L][n_theta][n_cols], i fastest, holding local columns i_first .. i_first + n_cols - 1; asynchronous on the
+ * stream; no boundary condition is applied by the write (never write a physical boundary column).  TEUK_EINVAL if the
+ * range leaves the handle's columns, TEUK_ESTATE before teuk_set_initial. */
+int teuk_read_columns_device(teuk_ctx *, int i_first, int n_cols, double *d_out);
+int teuk_write_columns_device(teuk_ctx *, int i_first, int n_cols, const double *d_in);
 
 /* Observer series: out[count][4][L] = Phi_R, Phi_I, Pi_R, Pi_I at the observer after each completed
  * iteration (sample k <-> t = (k+1) dt), count <= max_samples; synchronises.  Returns

@@ -18,6 +18,7 @@ struct SetupConsts {
     R4 tau_h, tau_f;         // dt/2, dt
     int s, m, n_r, n_theta, pitch;
     long plane;
+    int k0;                  // radial slab (NEXT-4): this handle's column 0 is global column k0/2; r*_k = rmin + (k0 + k) dr/2
 };
 
 MPX R4 q_tortoise(const SetupConsts& C, const R4& y, R4& delta_out, R4& r_out) {
@@ -36,7 +37,7 @@ __global__ void radial_kernel(SetupConsts C, double* __restrict__ r_tab, double*
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= 2 * C.n_r - 1) return;
     // r*_k = r*_min + k dr*/2
-    R4 rs = add(C.rmin, mul_d(scale2(C.dr, 0.5), (double)k));
+    R4 rs = add(C.rmin, mul_d(scale2(C.dr, 0.5), (double)(k + C.k0)));
     // fp64 Newton for the starting value
     double M = C.M.x[0], rp = C.rp.x[0], rpm = C.rpm.x[0], cp = C.cplus.x[0], cm = C.cminus.x[0], a = C.a.x[0];
     double rsd = rs.x[0];

@@ -76,6 +76,7 @@ static Layout make_layout(int n_r, int n_theta, int L, long cap) {
 struct teuk_ctx {
     double M, a, rmin, rmax, dt;
     int s, m, n_r, n_theta, L;
+    int i_lo = 0, n_r_global = 0;      // radial slab: local column i <-> global column i_lo + i
     long cap_alloc;
     char* ws;
     Layout lay;
@@ -251,10 +252,12 @@ static int launch_coef_any(teuk_ctx* c, int half, int fold, double* out) {
     return launch_coef<4>(c, half, fold, out);
 }
 
-extern "C" int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double rstar_min, double rstar_max,
-                           double dt, int precision, void* d_workspace, size_t workspace_bytes, long obs_capacity,
-                           void* cuda_stream, teuk_ctx** out) {
+// one handle = columns [i_lo, i_lo + n_r) of the uniform grid of n_r_global nodes on [rstar_min, rstar_max]
+static int create_impl(double M, double a, int s, int m, int n_r_global, int i_lo, int n_r, int n_theta, double rstar_min,
+                       double rstar_max, double dt, int precision, void* d_workspace, size_t workspace_bytes,
+                       long obs_capacity, void* cuda_stream, teuk_ctx** out) {
     if (!out || !d_workspace || !valid_sizes(n_r, n_theta, precision, obs_capacity)) return TEUK_EINVAL;
+    if (i_lo < 0 || (long)i_lo + n_r > n_r_global || n_r_global >= (1 << 29)) return TEUK_EINVAL;
     if (!(M > 0) || !(std::fabs(a) < M) || !(dt > 0) || !(rstar_min < rstar_max)) return TEUK_EINVAL;
     if (!std::isfinite(M) || !std::isfinite(a) || !std::isfinite(dt) || !std::isfinite(rstar_min) ||
         !std::isfinite(rstar_max))
@@ -265,6 +268,7 @@ extern "C" int teuk_create(double M, double a, int s, int m, int n_r, int n_thet
     if (!c) return TEUK_ENOMEM;
     c->M = M; c->a = a; c->s = s; c->m = m; c->n_r = n_r; c->n_theta = n_theta; c->L = precision;
     c->rmin = rstar_min; c->rmax = rstar_max; c->dt = dt; c->cap_alloc = obs_capacity;
+    c->i_lo = i_lo; c->n_r_global = n_r_global;
     c->ws = (char*)d_workspace; c->lay = lay; c->stream = (cudaStream_t)cuda_stream;
 
     // ---- host scalars in quad-double
@@ -279,7 +283,8 @@ extern "C" int teuk_create(double M, double a, int s, int m, int n_r, int n_thet
     C.cplus = div(mul(scale2(C.M, 2.0), C.rp), C.rpm);
     C.cminus = div(mul(scale2(C.M, 2.0), rm), C.rpm);
     C.rmin = from_double<4>(rstar_min);
-    C.dr = div(sub(from_double<4>(rstar_max), C.rmin), from_double<4>((double)(n_r - 1)));
+    C.dr = div(sub(from_double<4>(rstar_max), C.rmin), from_double<4>((double)(n_r_global - 1)));
+    C.k0 = 2 * i_lo;
     C.dth = div(qc.pi, from_double<4>((double)n_theta));
     C.ln2 = qc.ln2;
     C.tau_f = from_double<4>(dt);
@@ -349,6 +354,20 @@ extern "C" int teuk_create(double M, double a, int s, int m, int n_r, int n_thet
     return TEUK_OK;
 }
 
+extern "C" int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double rstar_min, double rstar_max,
+                           double dt, int precision, void* d_workspace, size_t workspace_bytes, long obs_capacity,
+                           void* cuda_stream, teuk_ctx** out) {
+    return create_impl(M, a, s, m, n_r, 0, n_r, n_theta, rstar_min, rstar_max, dt, precision, d_workspace, workspace_bytes,
+                       obs_capacity, cuda_stream, out);
+}
+
+extern "C" int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_theta, double rstar_min,
+                                double rstar_max, double dt, int precision, int i_lo, int n_win, void* d_workspace,
+                                size_t workspace_bytes, long obs_capacity, void* cuda_stream, teuk_ctx** out) {
+    return create_impl(M, a, s, m, n_r_global, i_lo, n_win, n_theta, rstar_min, rstar_max, dt, precision, d_workspace,
+                       workspace_bytes, obs_capacity, cuda_stream, out);
+}
+
 extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     if (!c || !key) return TEUK_EINVAL;
     if (c->have_init) return TEUK_ESTATE;
@@ -387,7 +406,7 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
 extern "C" int teuk_set_observer(teuk_ctx* c, double rstar_obs, double theta_obs, long capacity) {
     if (!c || capacity < 0 || capacity > c->cap_alloc || !std::isfinite(rstar_obs) || !std::isfinite(theta_obs))
         return TEUK_EINVAL;
-    R4 x = div(sub(from_double<4>(rstar_obs), c->C.rmin), c->C.dr);
+    R4 x = sub(div(sub(from_double<4>(rstar_obs), c->C.rmin), c->C.dr), from_double<4>((double)c->i_lo));
     R4 y = sub(div(from_double<4>(theta_obs), c->C.dth), from_double<4>(0.5));
     int i0 = (int)std::floor(x.x[0]), j0 = (int)std::floor(y.x[0]);
     if (x.x[0] < 0 || x.x[0] > c->n_r - 1 || y.x[0] < 0 || y.x[0] > c->n_theta - 1) return TEUK_EINVAL;
@@ -811,6 +830,36 @@ extern "C" int teuk_read(teuk_ctx* c, double* host_planes) {
     return TEUK_OK;
 }
 
+// halo strips of the current state: buf is double[4][L][n_theta][n_cols] (i fastest), columns i_first .. i_first + n_cols - 1
+__global__ void columns_kernel(double* __restrict__ state, double* __restrict__ buf, int i_first, int n_cols, int n_theta,
+                               int pitch, long plane, int planes, int write) {
+    long idx = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (idx >= (long)planes * n_theta * n_cols) return;
+    int ic = (int)(idx % n_cols);
+    long rest = idx / n_cols;
+    int j = (int)(rest % n_theta);
+    int pl = (int)(rest / n_theta);
+    long g = pl * plane + (long)j * pitch + i_first + ic;
+    if (write) state[g] = buf[idx];
+    else buf[idx] = state[g];
+}
+
+static int columns_io(teuk_ctx* c, int i_first, int n_cols, double* d_buf, int write) {
+    if (!c || !d_buf || i_first < 0 || n_cols < 1 || (long)i_first + n_cols > c->n_r) return TEUK_EINVAL;
+    if (!c->have_init) return TEUK_ESTATE;
+    long total = 4L * c->L * c->n_theta * n_cols;
+    columns_kernel<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(c->state(c->cur), d_buf, i_first, n_cols, c->n_theta,
+                                                                          c->lay.pitch, c->lay.plane, 4 * c->L, write);
+    c->launches++;
+    return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+}
+extern "C" int teuk_read_columns_device(teuk_ctx* c, int i_first, int n_cols, double* d_out) {
+    return columns_io(c, i_first, n_cols, d_out, 0);
+}
+extern "C" int teuk_write_columns_device(teuk_ctx* c, int i_first, int n_cols, const double* d_in) {
+    return columns_io(c, i_first, n_cols, const_cast<double*>(d_in), 1);
+}
+
 extern "C" int teuk_observe(teuk_ctx* c, double* host_out, long max_samples, long* count) {
     if (!c || !host_out || !count || max_samples < 0) return TEUK_EINVAL;
     long n = c->steps_done - c->series_origin;
@@ -895,7 +944,7 @@ static R4 q_fejer_weight(int j, int N, const R4& pi) {
 extern "C" int teuk_set_multipole_observer(teuk_ctx* c, double rstar_obs, int n_ell, long capacity) {
     if (!c || n_ell < 1 || n_ell > MP_MAX_ELL || capacity < 0 || capacity > c->cap_alloc || !std::isfinite(rstar_obs))
         return TEUK_EINVAL;
-    R4 x = div(sub(from_double<4>(rstar_obs), c->C.rmin), c->C.dr);
+    R4 x = sub(div(sub(from_double<4>(rstar_obs), c->C.rmin), c->C.dr), from_double<4>((double)c->i_lo));
     int i0 = (int)std::floor(x.x[0]);
     if (x.x[0] < 0 || x.x[0] > c->n_r - 1) return TEUK_EINVAL;
     if (i0 > c->n_r - 2) i0 = c->n_r - 2;

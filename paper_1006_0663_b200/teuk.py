@@ -27,6 +27,9 @@ SIGNATURES = {
     "teuk_workspace_bytes": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_long, C.POINTER(C.c_size_t)]),
     "teuk_create": (C.c_int, [C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
                               C.c_double, C.c_int, C.c_void_p, C.c_size_t, C.c_long, C.c_void_p, C.POINTER(_h)]),
+    "teuk_create_slab": (C.c_int, [C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                                   C.c_double, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_long, C.c_void_p,
+                                   C.POINTER(_h)]),
     "teuk_set_option": (C.c_int, [_h, C.c_char_p, C.c_double]),
     "teuk_set_observer": (C.c_int, [_h, C.c_double, C.c_double, C.c_long]),
     "teuk_set_initial": (C.c_int, [_h, _dp, C.c_int]),
@@ -34,6 +37,8 @@ SIGNATURES = {
     "teuk_step": (C.c_int, [_h, C.c_long]),
     "teuk_read": (C.c_int, [_h, _dp]),
     "teuk_read_device": (C.c_int, [_h, C.c_void_p]),
+    "teuk_read_columns_device": (C.c_int, [_h, C.c_int, C.c_int, C.c_void_p]),
+    "teuk_write_columns_device": (C.c_int, [_h, C.c_int, C.c_int, C.c_void_p]),
     "teuk_observe": (C.c_int, [_h, _dp, C.c_long, _lp]),
     "teuk_set_multipole_observer": (C.c_int, [_h, C.c_double, C.c_int, C.c_long]),
     "teuk_observe_multipoles": (C.c_int, [_h, _dp, C.c_long, _lp]),
@@ -82,12 +87,16 @@ class Teuk:
     """One solver handle (teuk_ctx).  Methods are 1:1 with the C calls."""
 
     def __init__(self, M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision, obs_capacity=0,
-                 device="cuda:0", stream=None):
+                 device="cuda:0", stream=None, slab=None):
+        """slab = (i_lo, n_win): teuk_create_slab, the handle holds that column range of the n_r-node grid"""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1006_0663_b200.teuk needs a CUDA device; there is no CPU fallback")
         self.torch = torch
-        self.n_r, self.n_theta, self.L = n_r, n_theta, precision
+        n_r_global, i_lo = n_r, 0
+        if slab is not None:
+            i_lo, n_r = int(slab[0]), int(slab[1])
+        self.n_r, self.n_theta, self.L, self.i_lo, self.n_r_global = n_r, n_theta, precision, i_lo, n_r_global
         nbytes = workspace_bytes(n_r, n_theta, precision, obs_capacity)
         self.device = torch.device(device)
         with torch.cuda.device(self.device):
@@ -97,9 +106,14 @@ class Teuk:
             base = self.workspace.data_ptr()
             self._ws_ptr = (base + 255) // 256 * 256
             self.h = _h()
-            _chk(lib.teuk_create(M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision,
-                                 C.c_void_p(self._ws_ptr), nbytes, obs_capacity,
-                                 C.c_void_p(self.stream.cuda_stream), C.byref(self.h)), "teuk_create")
+            if slab is None:
+                _chk(lib.teuk_create(M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision,
+                                     C.c_void_p(self._ws_ptr), nbytes, obs_capacity,
+                                     C.c_void_p(self.stream.cuda_stream), C.byref(self.h)), "teuk_create")
+            else:
+                _chk(lib.teuk_create_slab(M, a, s, m, n_r_global, n_theta, rstar_min, rstar_max, dt, precision, i_lo, n_r,
+                                          C.c_void_p(self._ws_ptr), nbytes, obs_capacity,
+                                          C.c_void_p(self.stream.cuda_stream), C.byref(self.h)), "teuk_create_slab")
 
     @classmethod
     def from_workload(cls, w, precision=None, obs_capacity=0, **kw):
@@ -158,6 +172,23 @@ class Teuk:
         _chk(lib.teuk_read_device(self.h, C.c_void_p(t.data_ptr())), "teuk_read_device")
         self.torch.cuda.current_stream(self.device).wait_stream(self.stream)   # consumers run there
         return t
+
+    def read_columns(self, i_first: int, n_cols: int, out=None):
+        """local columns i_first .. i_first + n_cols - 1 -> CUDA tensor [4][L][n_theta][n_cols]"""
+        if out is None:
+            out = self.torch.empty((4, self.L, self.n_theta, n_cols), dtype=self.torch.float64, device=self.device)
+        assert out.is_contiguous() and out.numel() == 4 * self.L * self.n_theta * n_cols
+        self.stream.wait_stream(self.torch.cuda.current_stream(self.device))     # `out` may still be in use there
+        _chk(lib.teuk_read_columns_device(self.h, i_first, n_cols, C.c_void_p(out.data_ptr())), "teuk_read_columns_device")
+        self.torch.cuda.current_stream(self.device).wait_stream(self.stream)
+        return out
+
+    def write_columns(self, i_first: int, t):
+        t = t.contiguous()
+        assert t.is_cuda and t.dtype == self.torch.float64 and tuple(t.shape[:3]) == (4, self.L, self.n_theta)
+        self.stream.wait_stream(self.torch.cuda.current_stream(self.device))     # t was produced there
+        _chk(lib.teuk_write_columns_device(self.h, i_first, t.shape[3], C.c_void_p(t.data_ptr())), "teuk_write_columns_device")
+        t.record_stream(self.stream)
 
     def observe(self, max_samples: int, allow_nonfinite=False):
         out = np.zeros((max(max_samples, 1), 4, self.L))
