@@ -35,6 +35,9 @@ def parse():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--no-extra", action="store_true", help="skip the dd/qd side measurements and the cpu baseline")
     ap.add_argument("--option", action="append", default=[], help="key=value passed to teuk_set_option")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: independent replicas (default, weak scaling) or ONE problem cut into r* slabs with a halo "
+                         "exchange per 32 iterations (NEXT-4, strong scaling; paper_1006_0663_b200/slabs.py)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json config 5: one JSON line per (N_r, N_theta, precision) cell")
     return ap.parse_args()
 
@@ -258,12 +261,93 @@ def run_sweep(args):
                 print(json.dumps(line), flush=True)
 
 
+def run_slabs(args):
+    """--shard slabs: the workload's grid cut into world_size r* slabs, one per GPU; each rank steps its window and swaps
+    halo strips with its neighbours (NCCL point-to-point) once per 32 iterations.  value = the WHOLE grid's updates / max
+    over ranks of the device time (strong scaling); redundant halo columns are not counted as updates."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1006_0663_b200 import inputs, replicas, slabs
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    d = None
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        d = dist
+    w = workload(args.workload)
+    every = 32
+    slab = slabs.plan(w.n_r, world, every)[rank]
+    opts = {k: float(v) for k, _, v in (o.partition("=") for o in args.option)}
+    u0 = np.ascontiguousarray(inputs.initial_state(w)[..., slab.wlo:slab.whi])
+    host_in = torch.from_numpy(u0).pin_memory()
+    host_out = torch.empty((4, w.precision, w.n_theta, slab.n_win), dtype=torch.float64).pin_memory()
+
+    def one_run(steps, through_host):
+        st = slabs.TeukStepper(w, slab, options=opts, device=f"cuda:{local}")
+        run = slabs.SlabRun(slab, st, d, exchange_every=every)
+        st.g.set_initial_pinned(host_in)
+        run.step(args.warmup)
+        torch.cuda.synchronize()
+        if d is not None:
+            d.barrier()
+        n0 = st.g.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        if through_host:
+            st.g.set_initial_pinned(host_in)
+        e0.record(st.g.stream)
+        run.step(steps)
+        e1.record(st.g.stream)                  # the last exchange ends with write_columns on this stream
+        if through_host:
+            st.g.read_pinned(host_out)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        res = (e0.elapsed_time(e1), wall, st.g.launch_count() - n0, st.g.step_geometry(), run.exchanges)
+        st.g.close()
+        return res
+
+    with ClockSampler(local) as cs:
+        ms, _, launches, geom, exch = one_run(args.steps, False)
+    _, wall, _, _, _ = one_run(args.steps, True)
+    points = float(w.n_r * w.n_theta)
+    # every rank reports its share of the grid's updates; aggregate() sums them and takes the max time
+    mine = float((slab.hi - slab.lo) * w.n_theta) * args.steps
+    ms_max, _, value = replicas.aggregate(ms, mine, d, device="cuda")
+    _, _, e2e_val = replicas.aggregate(wall * 1e3, mine, d, device="cuda")
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        L = w.precision
+        ach = ALG_BYTES_PER_UPDATE[L] * (slab.n_win * w.n_theta) / (ms / args.steps * 1e-3) / 1e9
+        print(json.dumps({
+            "metric": "Teukolsky grid-point updates/s", "value": value, "unit": "updates/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": {1: "f64", 2: "f64x2 (double-double)", 4: "f64x4 (quad-double)"}[L],
+            "data": "synthetic",
+            "config": {"workload": w.name, "n_r": w.n_r, "n_theta": w.n_theta, "precision_limbs": L,
+                       "parallelism": f"r*-slabs x{world}, halo {slab.halo}, one exchange per {every} iterations",
+                       "rank0_window_columns": slab.n_win, "geometry": geom, "halo_exchanges": exch,
+                       "l2": "per-rank working set shrinks with N; no flush (strong scaling of the named workload)"},
+            "clocks": cs.summary(),
+            "e2e": {"value": e2e_val, "unit": "updates/s", "h2d_bytes_per_step": host_in.numel() * 8 / args.steps,
+                    "d2h_bytes_per_step": host_out.numel() * 8 / args.steps},
+            "gpu_launches": launches,
+            "roofline": {"bound": "hbm" if L == 1 else "fp64 pipe (see profiles/)", "achieved": ach, "peak": peak, "unit": "GB/s",
+                         "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                         "note": "rank 0's window incl. halo columns"}}), flush=True)
+    if d is not None:
+        d.destroy_process_group()
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
     if args.sweep:
         return run_sweep(args)
+    if args.shard == "slabs":
+        return run_slabs(args)
     import torch
     import torch.distributed as dist
     rank = int(os.environ.get("RANK", "0"))
