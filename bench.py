@@ -38,6 +38,7 @@ def parse():
     ap.add_argument("--shard", default="replicas", choices=["replicas", "slabs"],
                     help="N > 1: independent replicas (default, weak scaling) or ONE problem cut into r* slabs with a halo "
                          "exchange per 32 iterations (NEXT-4, strong scaling; paper_1006_0663_b200/slabs.py)")
+    ap.add_argument("--precisions", default="", help="--sweep: comma-separated limb counts to run (default 1,2,4)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json config 5: one JSON line per (N_r, N_theta, precision) cell")
     return ap.parse_args()
 
@@ -242,7 +243,7 @@ def run_sweep(args):
     peak, _ = measured_peaks()
     pipe = teuk.bench_fp64("dadd")
     inst = {2: 1294.0, 4: 13320.0}
-    for L in (1, 2, 4):
+    for L in ((1, 2, 4) if not args.precisions else [int(x) for x in args.precisions.split(",")]):
         for nr in (4096, 16384, 65536):
             for nt in (32, 64, 256):
                 w = workload(f"sweep:{nr}x{nt}:{L}")
@@ -253,7 +254,10 @@ def run_sweep(args):
                         "dt_over_dr": w.dt / w.dr, "updates_per_s": ups, "ms_per_step": ms / steps, "finite": finite,
                         "geometry": geom}
                 if L == 1:
-                    line["roofline"] = {"bound": "hbm", "frac": ups * 192.0 / 1e9 / peak, "peak_gbs": peak,
+                    opt = [o.replace(" ", "") for o in args.option]
+                    bpu = 80.0 if "coef_variant=1" in opt else 96.0 if "time_block=2" in opt else 192.0
+                    line["roofline"] = {"bound": "hbm", "frac": ups * bpu / 1e9 / peak, "peak_gbs": peak,
+                                        "algorithmic_bytes_per_update": bpu,
                                         "working_set_mib": 24 * nr * nt * 8 // 2 ** 20}
                 else:
                     line["roofline"] = {"bound": "fp64 pipe", "frac": ups * inst[L] / pipe, "peak_inst_per_s": pipe,

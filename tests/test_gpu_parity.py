@@ -524,19 +524,20 @@ def test_config2_prefix_full_grid_fp64(teuk):
                            "(measured on B200: Phi 2.1e-14, Pi 8.9e-13, observer 2.8e-14; DESIGN.md section 5)")
 def test_config2_full_length_fp64(teuk):
     """BASELINE.json config 2 at full size AND full length (20000 steps) against the full-grid oracle,
-    for both coefficient supplies (stored planes; semi-recompute)."""
+    for both coefficient supplies (stored planes; semi-recompute) and the two-iterations-per-launch kernel."""
     w = inputs.config(2)
     u0 = inputs.initial_state(w)
     o = run_oracle(w, u0, w.steps, observer=w.observer)
     ref, sref = o.read(), o.observe(w.steps)
     res = {}
-    for cv in (0, 1):
-        g = run_gpu(teuk, w, u0, w.steps, observer=w.observer, options={"coef_variant": cv})
-        res[cv] = (oracle.rel_linf(g.read(), ref), series_err(g.observe(w.steps), sref))
-        print("cfg2 full length, coef_variant", cv, ": state", res[cv][0], "observer", res[cv][1])
-    for cv in (0, 1):
-        assert max(res[cv][0].values()) <= TOL[1], cv
-        assert max(res[cv][1].values()) <= TOL[1], cv
+    variants = {"stored planes": {"coef_variant": 0}, "semi-recompute": {"coef_variant": 1}, "time_block=2": {"time_block": 2}}
+    for name, opts in variants.items():
+        g = run_gpu(teuk, w, u0, w.steps, observer=w.observer, options=opts)
+        res[name] = (oracle.rel_linf(g.read(), ref), series_err(g.observe(w.steps), sref))
+        print("cfg2 full length,", name, ": state", res[name][0], "observer", res[name][1])
+    for name in variants:
+        assert max(res[name][0].values()) <= TOL[1], name
+        assert max(res[name][1].values()) <= TOL[1], name
 
 
 @pytest.mark.parametrize("cfg", [3, 4])
