@@ -568,6 +568,29 @@ def test_full_length_precision_ladder_on_gpu(teuk, cfg):
     assert max(e24.values()) > 0 and max(e12.values()) > 1e-18          # the rungs are distinct
 
 
+@pytest.mark.skipif(os.environ.get("TEUK_FULL_LENGTH") != "1",
+                    reason="15 minutes of host time for the full-grid dd / qd oracle; set TEUK_FULL_LENGTH=1 "
+                           "(TEUK_FULL_STEPS_CFG3 / TEUK_FULL_STEPS_CFG4 change the prefix; results: DESIGN.md section 5)")
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_config3_config4_full_grid_long_runs(teuk, cfg):
+    """BASELINE.json configs 3 (dd) and 4 (qd) at FULL size against the FULL-GRID oracle (no windows), observer series
+    included, over a prefix: the exact-then-round oracle advances about 3.5e5 dd or qd updates/s on 16 cores (3 s per
+    iteration of config 3), so the full 20000 / 50000 steps would take 17 / 11 hours; the rest of the run stays covered
+    by the full-size windowed tests and the full-length precision ladder."""
+    w = inputs.config(cfg)
+    steps = int(os.environ.get(f"TEUK_FULL_STEPS_CFG{cfg}", {3: 200, 4: 400}[cfg]))
+    u0 = inputs.initial_state(w)
+    g = run_gpu(teuk, w, u0, steps, observer=w.observer)
+    got, ser = g.read(), g.observe(steps)
+    g.close()
+    o = run_oracle(w, u0, steps, observer=w.observer)
+    err = oracle.rel_linf(got, o.read())
+    serr = series_err(ser, o.observe(steps))
+    print("cfg", cfg, "full grid,", steps, "steps: state", err, "observer", serr)
+    assert max(err.values()) <= TOL[w.precision]
+    assert max(serr.values()) <= TOL[w.precision]
+
+
 # ------------------------------------------------------------------------------- invariants and edge cases
 @pytest.mark.parametrize("L", [1, 2, 4])
 def test_gpu_exact_invariants(teuk, L):
