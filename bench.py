@@ -255,7 +255,7 @@ def run_sweep(args):
                         "geometry": geom}
                 if L == 1:
                     opt = [o.replace(" ", "") for o in args.option]
-                    bpu = 80.0 if "coef_variant=1" in opt else 96.0 if "time_block=2" in opt else 192.0
+                    bpu = 80.0 if "coef_variant=1" in opt else 64.0 if "coef_variant=2" in opt else 96.0 if "time_block=2" in opt else 192.0
                     line["roofline"] = {"bound": "hbm", "frac": ups * bpu / 1e9 / peak, "peak_gbs": peak,
                                         "algorithmic_bytes_per_update": bpu,
                                         "working_set_mib": 24 * nr * nt * 8 // 2 ** 20}
@@ -380,8 +380,11 @@ def main():
             d.destroy_process_group()
         return
     peak, peak_src = measured_peaks()
-    recompute = any(o.replace(" ", "") == "coef_variant=1" for o in args.option)
-    bytes_per_update = 80.0 if recompute else ALG_BYTES_PER_UPDATE[L]     # H1b variant (b): state 64 B + two 1/Sigma planes 16 B
+    opt_set = {o.replace(" ", "") for o in args.option}
+    recompute = "coef_variant=1" in opt_set or "coef_variant=2" in opt_set
+    # H1b variant (b): state 64 B + two 1/Sigma planes 16 B; (c): state only; NEXT-3: half of the stored-plane traffic
+    bytes_per_update = (80.0 if "coef_variant=1" in opt_set else 64.0 if "coef_variant=2" in opt_set
+                        else 96.0 if "time_block=2" in opt_set and L == 1 else ALG_BYTES_PER_UPDATE[L])
     alg_bytes = bytes_per_update * points
     achieved = alg_bytes / (ms / args.steps * 1e-3) / 1e9
     line = {
@@ -401,7 +404,7 @@ def main():
                         "state once per K-step call divided by K"},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": load_traffic(f"{w.name}"), "peak_source": peak_src, "kernel": "step_kernel_f64_rc" if recompute else ("step_kernel_f64_tma" if L == 1 else f"step_kernel<{L}>"),
+                     "traffic": load_traffic(f"{w.name}"), "peak_source": peak_src, "kernel": "step_kernel_f64_rc" if recompute else ("step2_kernel_f64_tma" if "time_block=2" in opt_set and L == 1 else "step_kernel_f64_tma" if L == 1 else f"step_kernel<{L}>"),
                      "algorithmic_bytes_per_update": bytes_per_update},
     }
     if not args.no_extra and world == 1:
@@ -428,6 +431,11 @@ def main():
             ach = 80.0 * points / (msr / args.steps * 1e-3) / 1e9
             line["semi_recompute"] = {"updates_per_s": points * args.steps / (msr * 1e-3), "ms_per_step": msr / args.steps,
                                       "algorithmic_bytes_per_update": 80.0, "hbm_frac": ach / peak, "geometry": gr, "finite": fr}
+            # H1b variant (c): full recompute (1/Sigma by rsqrt per point; state-only traffic, 64 B/update)
+            msf, lf, gf, ff = time_device(torch, teuk, w, args.steps, args.warmup, list(args.option) + ["coef_variant=2"])
+            achf = 64.0 * points / (msf / args.steps * 1e-3) / 1e9
+            line["full_recompute"] = {"updates_per_s": points * args.steps / (msf * 1e-3), "ms_per_step": msf / args.steps,
+                                      "algorithmic_bytes_per_update": 64.0, "hbm_frac": achf / peak, "geometry": gf, "finite": ff}
             # NEXT-3: two iterations per launch (u^{n+1} and the coefficient tiles stay on the SM): 96 B/update
             mst, lt, gt, ft = time_device(torch, teuk, w, args.steps, args.warmup, list(args.option) + ["time_block=2"])
             acht = 96.0 * points / (mst / args.steps * 1e-3) / 1e9

@@ -55,7 +55,8 @@ int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_the
 /* Options, only before teuk_set_initial (else TEUK_ESTATE): "graph_steps" (even, >= 2; steps per
  * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic), "use_tma" (fp64: 1 = TMA
  * kernel, default; 0 = generic kernel), "variant" (dd/qd launch shape 0..2), "coef_variant" (0 = precomputed
- * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only),
+ * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only; 2 = full recompute:
+ * 1-D tables only, 1/Sigma = rsqrt(R^2 - a^2 Delta sin^2 theta) per point, fp64 only),
  * "pdl" (fp64 TMA kernels: 1 = programmatic dependent launch, the next step prefetches its half-step coefficient
  * tile while the current one drains; default 0, measured neutral), "theta_order" (2 = second-order centred theta differences, default; 10 = the 10th-order
  * 11-point operator of PAPER.md:126, needs n_theta >= 5), "time_block" (1 = one iteration per launch, default; 2 = two

@@ -10,10 +10,10 @@ const void* tma_step_fn(int ti, int tj) {
     if (tj == 16) return (const void*)step_kernel_f64_tma<32, 16>;
     return nullptr;
 }
-const void* rc_step_fn(int ti, int tj) {
+const void* rc_step_fn(int ti, int tj, int full) {
     if (ti != 32) return nullptr;
-    if (tj == 8) return (const void*)step_kernel_f64_rc<32, 8>;
-    if (tj == 16) return (const void*)step_kernel_f64_rc<32, 16>;
+    if (tj == 8) return full ? (const void*)step_kernel_f64_rc<32, 8, true> : (const void*)step_kernel_f64_rc<32, 8, false>;
+    if (tj == 16) return full ? (const void*)step_kernel_f64_rc<32, 16, true> : (const void*)step_kernel_f64_rc<32, 16, false>;
     return nullptr;
 }
 const void* col_tma_fn(int ti) {

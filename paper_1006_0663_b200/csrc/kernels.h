@@ -16,7 +16,7 @@ const void* generic_col_fn_2(int* threads);
 const void* generic_col_fn_4(int* threads);
 // fp64 TMA kernels (step_kernel_tma.cuh): stored planes, semi-recompute, 10th-order column kernel
 const void* tma_step_fn(int ti, int tj);
-const void* rc_step_fn(int ti, int tj);
+const void* rc_step_fn(int ti, int tj, int full);     // full = H1b variant (c)
 const void* col_tma_fn(int ti);
 // fp64 two-iterations-per-launch kernel (step_kernel_tb2.cuh, NEXT-3)
 const void* tb2_step_fn(int ti, int tj);

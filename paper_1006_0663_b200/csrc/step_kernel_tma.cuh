@@ -230,7 +230,11 @@ __device__ __forceinline__ void rc_eval(RcCoef& o, double isig, const double* rt
     o.c[7] = q * rt[13 * stride];
 }
 
-template <int TI, int TJ>
+// FULL = H1b variant (c), full recompute: the 1/Sigma planes are not read either; 1/Sigma = rsqrt(R^2 - a^2 Delta sin^2 theta)
+// (Eq. 7) per point and sub-step from the two spare r-tables (R^2, a^2 Delta) and sin^2 theta.  State-only
+// HBM traffic: 64 B/update.  fp64 rsqrt of a sum of two rounded table entries instead of a quad-double evaluation rounded
+// once: the coefficients differ from the stored planes by a few more ulps (tested), no cancellation (a^2 Delta sin^2 <= 0.06 R^2).
+template <int TI, int TJ, bool FULL>
 __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant__ CUtensorMap tm_u,
                                                          const __grid_constant__ CUtensorMap tm_ish,
                                                          const __grid_constant__ CUtensorMap tm_isi,
@@ -261,8 +265,8 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
         mbar_init(&bar[2], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        mbar_expect_tx(&bar[2], HR * CC * 8 + NT * CC * 8);
-        tma_load_3d(ish, &tm_ish, i0 - 2, j0 - 1, 0, &bar[2]);
+        mbar_expect_tx(&bar[2], (FULL ? 0 : HR * CC * 8) + NT * CC * 8);
+        if (!FULL) tma_load_3d(ish, &tm_ish, i0 - 2, j0 - 1, 0, &bar[2]);
         tma_load_3d(rth, &tm_rth, i0 - 2, 0, 0, &bar[2]);
     }
     if (tid < 4 * (TJ + 2)) {
@@ -274,8 +278,8 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
     if (tid == 0) {
         mbar_expect_tx(&bar[0], 4 * UR * UC * 8);
         tma_load_3d(us, &tm_u, i0 - 2, j0 - 2, 0, &bar[0]);
-        mbar_expect_tx(&bar[1], TJ * TI * 8 + NT * TI * 8);
-        tma_load_3d(isi, &tm_isi, i0, j0, 0, &bar[1]);
+        mbar_expect_tx(&bar[1], (FULL ? 0 : TJ * TI * 8) + NT * TI * 8);
+        if (!FULL) tma_load_3d(isi, &tm_isi, i0, j0, 0, &bar[1]);
         tma_load_3d(rti, &tm_rti, i0, 0, 0, &bar[1]);
     }
     __syncthreads();
@@ -297,7 +301,8 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
                 R1 cjv;
                 cjv.x[0] = tht[0][tr];
                 RcCoef cf;
-                rc_eval(cf, ish[tr * CC + tc + 1], rth + tc + 1, CC, tht[1][tr], tht[2][tr], tht[3][tr]);
+                const double is_h = FULL ? rsqrt(fma(-rth[15 * CC + tc + 1], tht[1][tr], rth[14 * CC + tc + 1])) : ish[tr * CC + tc + 1];
+                rc_eval(cf, is_h, rth + tc + 1, CC, tht[1][tr], tht[2][tr], tht[3][tr]);
                 R1 out[4];
                 substep<1>(ut, jh, rm, rp, sm, sp, tc + 1, tc + 2, cf, cjv, P.tq_half, true, out, out);
 #pragma unroll
@@ -332,7 +337,8 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
             R1 cjv;
             cjv.x[0] = tht[0][tr + 1];
             RcCoef cf;
-            rc_eval(cf, isi[tr * TI + tc], rti + tc, TI, tht[1][tr + 1], tht[2][tr + 1], tht[3][tr + 1]);
+            const double is_i = FULL ? rsqrt(fma(-rti[15 * TI + tc], tht[1][tr + 1], rti[14 * TI + tc])) : isi[tr * TI + tc];
+            rc_eval(cf, is_i, rti + tc, TI, tht[1][tr + 1], tht[2][tr + 1], tht[3][tr + 1]);
             substep<1>(ht, j, rm, rp, sm, sp, tc, tc + 1, cf, cjv, P.tq_full, false, bs, out);
         }
         long g = (long)j * P.pitch + i;

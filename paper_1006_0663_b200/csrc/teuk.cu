@@ -387,7 +387,7 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
         if ((v != 2 && v != 10) || c->n_theta < v / 2) return TEUK_EINVAL;
         c->theta_order = v;
     } else if (!strcmp(key, "coef_variant")) {
-        if (v < 0 || v > 1 || (v == 1 && c->L != 1)) return TEUK_EINVAL;
+        if (v < 0 || v > 2 || (v >= 1 && c->L != 1)) return TEUK_EINVAL;
         c->coef_variant = v;
     } else if (!strcmp(key, "variant")) {
         if (v < 0 || v > 2) return TEUK_EINVAL;
@@ -498,7 +498,7 @@ template <int TI, int TJ> static bool setup_rc(teuk_ctx* c) {
               make_map(&c->tm_rti, rt0, c->n_r, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, TI, RC_NT, 1) &&
               make_map(&c->tm_rth, rt0 + (size_t)RC_NT * y.pitch, c->n_r - 1, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, G::CC, RC_NT, 1);
     if (!ok) return false;
-    const void* fn = rc_step_fn(TI, TJ);
+    const void* fn = rc_step_fn(TI, TJ, c->coef_variant == 2);
     if (!fn || cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, G::TOTAL) != cudaSuccess) return false;
     c->ti = TI; c->tj = TJ; c->smem = G::TOTAL; c->threads = 256;
     c->grid = dim3((c->n_r + TI - 1) / TI, (c->n_theta + TJ - 1) / TJ);
@@ -580,7 +580,7 @@ static int choose_geometry(teuk_ctx* c) {
         const void* fn = col_fn(c, &c->threads);
         return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
     }
-    if (c->L == 1 && c->coef_variant == 1) {
+    if (c->L == 1 && c->coef_variant >= 1) {
         bool ok = (c->opt_tj == 8) ? setup_rc<32, 8>(c) : setup_rc<32, 16>(c);
         cudaGetLastError();
         if (!ok) return TEUK_ECUDA;       // the recompute variant exists only as a TMA kernel
@@ -661,7 +661,7 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         RcParams Q{c->dptr(c->lay.rc_th)};
         if (c->use_rc) {
             void* args[] = {&c->tm_state[from], &c->tm_ish, &c->tm_isi, &c->tm_rth, &c->tm_rti, &P, &Q};
-            le = cudaLaunchKernelExC(&cfg, rc_step_fn(c->ti, c->tj), args);
+            le = cudaLaunchKernelExC(&cfg, rc_step_fn(c->ti, c->tj, c->coef_variant == 2), args);
         } else {
             void* args[] = {&c->tm_state[from], &c->tm_ch, &c->tm_ci, &P};
             le = cudaLaunchKernelExC(&cfg, tma_step_fn(c->ti, c->tj), args);
@@ -1044,27 +1044,29 @@ extern "C" int teuk_get_tables(teuk_ctx* c, int half, double* host_out) {
 
 // test hook: recomputed folded coefficients of one family written as 8 planes [n_theta][pitch]
 __global__ void rc_tables_kernel(const double* __restrict__ isig, const double* __restrict__ rt, const double* __restrict__ th,
-                                 int cols, int n_theta, int pitch, long plane, double* __restrict__ out) {
+                                 int cols, int n_theta, int pitch, long plane, double* __restrict__ out, int full) {
     int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
     if (i >= cols) return;
     RcCoef cf;
-    rc_eval(cf, isig[(long)j * pitch + i], rt + i, pitch, th[j], th[n_theta + j], th[2 * n_theta + j]);
+    // full = variant (c): 1/Sigma from the R^2 and a^2 Delta tables, exactly as step_kernel_f64_rc<.., true> forms it
+    double is = full ? rsqrt(fma(-rt[15 * pitch + i], th[j], rt[14 * pitch + i])) : isig[(long)j * pitch + i];
+    rc_eval(cf, is, rt + i, pitch, th[j], th[n_theta + j], th[2 * n_theta + j]);
     for (int q = 0; q < 8; ++q) out[q * plane + (long)j * pitch + i] = cf.c[q];
 }
 
 extern "C" int teuk_get_folded(teuk_ctx* c, int half, int coef_variant, double* host_out) {
-    if (!c || !host_out || c->L != 1 || coef_variant < 0 || coef_variant > 1) return TEUK_EINVAL;
+    if (!c || !host_out || c->L != 1 || coef_variant < 0 || coef_variant > 2) return TEUK_EINVAL;
     int rows = half ? c->n_r - 1 : c->n_r;
     size_t n = (size_t)8 * c->lay.plane;
     std::vector<double> h(n);
     const double* src = c->dptr(half ? c->lay.coef_h : c->lay.coef_i);
     double* tmp = nullptr;
-    if (coef_variant == 1) {
+    if (coef_variant >= 1) {
         if (cudaMalloc(&tmp, n * 8) != cudaSuccess) return TEUK_ENOMEM;
         rc_tables_kernel<<<dim3((rows + 127) / 128, c->n_theta), 128, 0, c->stream>>>(
             c->dptr(c->lay.rc_isig) + (size_t)(half ? 1 : 0) * c->lay.plane,
             c->dptr(c->lay.rc_rt) + (size_t)(half ? 1 : 0) * RC_NT * c->lay.pitch, c->dptr(c->lay.rc_th), rows, c->n_theta,
-            c->lay.pitch, c->lay.plane, tmp);
+            c->lay.pitch, c->lay.plane, tmp, coef_variant == 2);
         src = tmp;
     }
     cudaError_t e = cudaMemcpyAsync(h.data(), src, n * 8, cudaMemcpyDeviceToHost, c->stream);

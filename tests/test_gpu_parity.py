@@ -250,6 +250,11 @@ def test_recomputed_coefficients_match_stored_planes(teuk, cfg):
         scale = np.abs(a).max(axis=0, keepdims=True)
         rel = np.abs(a - b) / np.maximum(np.abs(a), scale / 16)
         assert rel.max() <= 16 * 2.0 ** -52, (half, float(rel.max()), np.unravel_index(rel.argmax(), rel.shape))
+        # variant (c), full recompute: 1/Sigma = rsqrt(R^2 - a^2 Delta sin^2 theta) in fp64 enters up to the third power
+        c = g.folded(half, 2)
+        relc = np.abs(a - c) / np.maximum(np.abs(a), scale / 16)
+        print("cfg", cfg, "half", half, "max ulps (b)", float(rel.max()) * 2.0 ** 52, "(c)", float(relc.max()) * 2.0 ** 52)
+        assert relc.max() <= 32 * 2.0 ** -52, (half, float(relc.max()), np.unravel_index(relc.argmax(), relc.shape))
 
 
 @pytest.mark.parametrize("n_r,n_t,base", [(203, 13, 2), (512, 16, 1), (1000, 70, 2), (40, 3, 2)])
@@ -259,7 +264,7 @@ def test_recompute_kernel_parity_fp64(teuk, n_r, n_t, base):
     u0 = inputs.random_state(n_r, n_t, 1, seed=33)
     o = run_oracle(w, u0, 200, observer=(10.3, 1.1))
     ref, sref = o.read(), o.observe(200)
-    for opts in ({"coef_variant": 1}, {"coef_variant": 1, "tile_j": 8}):
+    for opts in ({"coef_variant": 1}, {"coef_variant": 1, "tile_j": 8}, {"coef_variant": 2}, {"coef_variant": 2, "tile_j": 8}):
         g = run_gpu(teuk, w, u0, 200, options=opts, observer=(10.3, 1.1))
         err = oracle.rel_linf(g.read(), ref)
         serr = series_err(g.observe(200), sref)
@@ -271,11 +276,12 @@ def test_recompute_kernel_config2_prefix(teuk):
     w = inputs.config(2)
     u0 = inputs.initial_state(w)
     steps = 1000
-    g = run_gpu(teuk, w, u0, steps, options={"coef_variant": 1})
     o = run_oracle(w, u0, steps)
-    err = oracle.rel_linf(g.read(), o.read())
-    print("cfg2 1000-step prefix, recompute supply:", err)
-    assert max(err.values()) <= TOL[1]
+    for cv in (1, 2):
+        g = run_gpu(teuk, w, u0, steps, options={"coef_variant": cv})
+        err = oracle.rel_linf(g.read(), o.read())
+        print("cfg2 1000-step prefix, recompute supply", cv, ":", err)
+        assert max(err.values()) <= TOL[1]
     with pytest.raises(teuk.TeukError):
         teuk.Teuk.from_workload(inputs.config(3).scaled(n_r=64)).set_option("coef_variant", 1)   # fp64 only
 
@@ -530,7 +536,8 @@ def test_config2_full_length_fp64(teuk):
     o = run_oracle(w, u0, w.steps, observer=w.observer)
     ref, sref = o.read(), o.observe(w.steps)
     res = {}
-    variants = {"stored planes": {"coef_variant": 0}, "semi-recompute": {"coef_variant": 1}, "time_block=2": {"time_block": 2}}
+    variants = {"stored planes": {"coef_variant": 0}, "semi-recompute": {"coef_variant": 1}, "full recompute": {"coef_variant": 2},
+                "time_block=2": {"time_block": 2}}
     for name, opts in variants.items():
         g = run_gpu(teuk, w, u0, w.steps, observer=w.observer, options=opts)
         res[name] = (oracle.rel_linf(g.read(), ref), series_err(g.observe(w.steps), sref))
