@@ -212,6 +212,14 @@ template <int TI, int TJ> struct RcGeom {
     static constexpr int TOTAL = US_B + ISH_B + ISI_B + RTH_B + RTI_B + HS_B + 128;
 };
 
+// 1/sqrt(x) for variant (c): hardware rsqrt (<= 1 ulp) plus one FMA Newton step, so the result is within ~0.5 ulp like
+// the stored 1/Sigma plane (the coefficient error is systematic and accumulates linearly over a long run)
+__device__ __forceinline__ double rsqrt_refined(double x) {
+    double y = rsqrt(x);
+    double e = fma(-(x * y), y, 1.0);
+    return fma(0.5 * y, e, y);
+}
+
 struct RcCoef {
     double c[8];
     __device__ __forceinline__ R1 get(int q) const { R1 r; r.x[0] = c[q]; return r; }
@@ -301,7 +309,7 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
                 R1 cjv;
                 cjv.x[0] = tht[0][tr];
                 RcCoef cf;
-                const double is_h = FULL ? rsqrt(fma(-rth[15 * CC + tc + 1], tht[1][tr], rth[14 * CC + tc + 1])) : ish[tr * CC + tc + 1];
+                const double is_h = FULL ? rsqrt_refined(fma(-rth[15 * CC + tc + 1], tht[1][tr], rth[14 * CC + tc + 1])) : ish[tr * CC + tc + 1];
                 rc_eval(cf, is_h, rth + tc + 1, CC, tht[1][tr], tht[2][tr], tht[3][tr]);
                 R1 out[4];
                 substep<1>(ut, jh, rm, rp, sm, sp, tc + 1, tc + 2, cf, cjv, P.tq_half, true, out, out);
@@ -337,7 +345,7 @@ __global__ void __launch_bounds__(256) step_kernel_f64_rc(const __grid_constant_
             R1 cjv;
             cjv.x[0] = tht[0][tr + 1];
             RcCoef cf;
-            const double is_i = FULL ? rsqrt(fma(-rti[15 * TI + tc], tht[1][tr + 1], rti[14 * TI + tc])) : isi[tr * TI + tc];
+            const double is_i = FULL ? rsqrt_refined(fma(-rti[15 * TI + tc], tht[1][tr + 1], rti[14 * TI + tc])) : isi[tr * TI + tc];
             rc_eval(cf, is_i, rti + tc, TI, tht[1][tr + 1], tht[2][tr + 1], tht[3][tr + 1]);
             substep<1>(ht, j, rm, rp, sm, sp, tc, tc + 1, cf, cjv, P.tq_full, false, bs, out);
         }

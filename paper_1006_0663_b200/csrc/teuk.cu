@@ -1049,7 +1049,7 @@ __global__ void rc_tables_kernel(const double* __restrict__ isig, const double* 
     if (i >= cols) return;
     RcCoef cf;
     // full = variant (c): 1/Sigma from the R^2 and a^2 Delta tables, exactly as step_kernel_f64_rc<.., true> forms it
-    double is = full ? rsqrt(fma(-rt[15 * pitch + i], th[j], rt[14 * pitch + i])) : isig[(long)j * pitch + i];
+    double is = full ? rsqrt_refined(fma(-rt[15 * pitch + i], th[j], rt[14 * pitch + i])) : isig[(long)j * pitch + i];
     rc_eval(cf, is, rt + i, pitch, th[j], th[n_theta + j], th[2 * n_theta + j]);
     for (int q = 0; q < 8; ++q) out[q * plane + (long)j * pitch + i] = cf.c[q];
 }
