@@ -11,25 +11,42 @@ import time
 import numpy as np
 
 
-def main(argv):
+def run(prec: int = 4, order: int = 10, t_end: float = 1080.0, n_ell: int = 9):
+    """-> (t[steps], a[steps][n_ell]) : leading limb of Re a_l'(t) at the config-4 observer, and the wall time of the run"""
     import torch
     from . import inputs, teuk
-    prec = int(argv[1]) if len(argv) > 1 else 4
-    order = int(argv[2]) if len(argv) > 2 else 10
     w = inputs.config(4).scaled(precision=prec)
     if order == 10:
         w = w.scaled(dt_override=0.5 * w.dt)
-    steps = int(1080.0 / w.dt)
+    steps = int(t_end / w.dt)
     g = teuk.Teuk.from_workload(w, obs_capacity=steps)
     g.set_option("theta_order", order)
-    g.set_multipole_observer(w.rstar_obs, 9, steps)
+    g.set_multipole_observer(w.rstar_obs, n_ell, steps)
     g.set_initial(inputs.initial_state(w))
     t0 = time.time()
     g.step(steps)
     torch.cuda.synchronize()
-    print(f"precision limbs {prec}, theta_order {order}: {steps} steps of {w.n_r} x {w.n_theta} in {time.time() - t0:.2f} s")
-    amp = g.observe_multipoles(steps)[:, :, 0, 0]
-    t = (np.arange(steps) + 1) * w.dt
+    wall = time.time() - t0
+    amp = g.observe_multipoles(steps)[:, :, 0, 0].copy()
+    g.close()
+    return (np.arange(steps) + 1) * w.dt, amp, wall, w
+
+
+def power_index(t, y, lo, hi):
+    """local power-law index d ln|y| / d ln t over lo < t < hi (None if y changes sign or vanishes there)"""
+    sel = (t > lo) & (t < hi)
+    a = np.abs(y[sel])
+    if a.min() <= 0 or np.any(np.sign(y[sel]) != np.sign(y[sel][0])):
+        return None
+    return float(np.polyfit(np.log(t[sel]), np.log(a), 1)[0])
+
+
+def main(argv):
+    prec = int(argv[1]) if len(argv) > 1 else 4
+    order = int(argv[2]) if len(argv) > 2 else 10
+    t, amp, wall, w = run(prec, order)
+    steps = len(t)
+    print(f"precision limbs {prec}, theta_order {order}: {steps} steps of {w.n_r} x {w.n_theta} in {wall:.2f} s")
     for lo, hi in ((400, 700), (700, 1050)):
         sel = (t > lo) & (t < hi)
         idx = []
@@ -39,7 +56,6 @@ def main(argv):
         print(f"local power index d ln|a_l'| / d ln t for t in [{lo}, {hi}], l' = 0..8: {idx}")
     k = int(np.searchsorted(t, 1000.0))
     print("a_l'(t = 1000), l' = 0..8:", ["%.3e" % v for v in amp[k]])
-    g.close()
 
 
 if __name__ == "__main__":

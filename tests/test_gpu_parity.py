@@ -602,6 +602,27 @@ def test_config3_config4_full_grid_long_runs(teuk, cfg):
     assert max(serr.values()) <= TOL[w.precision]
 
 
+def test_fig1_tail_rule_on_gpu(teuk):
+    """The paper's Fig. 1 experiment on the product path (quad-double, 10th-order theta operator, multipole observer;
+    BASELINE.json config 4 = Kerr a = 0.5, pure l = 0 data): the multipoles l' = 0 and 2 decay as t^-(l + l' + 3), the
+    rule the caption of Fig. 1 states (expected exponents from tests/golden/tail_exponents.txt), while the
+    SAME run in fp64 loses l' = 2 in rounding noise - the paper's case for high precision."""
+    from paper_1006_0663_b200 import fig1_tails
+    rows = [ln.split() for ln in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "tail_exponents.txt"))
+            if ln.strip() and not ln.startswith("#")]
+    n = {int(r[2]): int(r[3]) for r in rows if r[0] == "kerr" and r[1] == "0"}
+    t, amp, wall, w = fig1_tails.run(4, 10, t_end=1060.0, n_ell=3)
+    i0 = fig1_tails.power_index(t, amp[:, 0], 700, 1050)
+    i2 = fig1_tails.power_index(t, amp[:, 2], 700, 1050)
+    print("fig. 1 run, qd:", wall, "s; indices l'=0:", i0, "l'=2:", i2)
+    assert i0 is not None and abs(i0 + n[0]) < 0.1                 # -3
+    assert i2 is not None and abs(i2 + n[2]) < 0.4                 # -5 (still approaching the asymptote at t ~ 1000 M)
+    k = int(np.searchsorted(t, 1000.0))
+    assert 1e-13 < abs(amp[k, 2]) < 1e-9 and abs(amp[k, 1]) < 1e-40 * abs(amp[k, 0])     # odd l' stays at rounding level
+    t1, amp1, _, _ = fig1_tails.run(1, 10, t_end=1060.0, n_ell=3)
+    assert abs(amp1[k, 2]) > 100 * abs(amp[k, 2])                  # fp64: l' = 2 drowned in rounding noise
+
+
 # ------------------------------------------------------------------------------- invariants and edge cases
 @pytest.mark.parametrize("L", [1, 2, 4])
 def test_gpu_exact_invariants(teuk, L):
