@@ -251,13 +251,26 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel(StepParams P) {
     if (PF && v) load_coef(cc, P.coef_h, P.plane, (long)gj * P.pitch + gi);
 
     // ---- phase 0: stage the u^n tile (+1 column, +2 rows of halo); outside the grid -> 0
-    for (int k = tid; k < 4 * L * UR * UC; k += nth) {
-        int c = k % UC, rest = k / UC;
-        int r = rest % UR, pl = rest / UR;
-        int ui = iu0 + c, uj = ju0 + r;
-        double val = 0.0;
-        if (ui >= 0 && ui < nr && uj >= 0 && uj < nt) val = __ldg(P.u_in + pl * P.plane + (long)uj * P.pitch + ui);
-        us[k] = val;
+    //      (loads issued in batches of STG before any of them is stored: one round trip to L2/HBM per batch instead of
+    //      one per element - the unbatched loop was the largest long-scoreboard stall of the dd kernel)
+    constexpr int STG = 8;
+    const int n_stage = 4 * L * UR * UC;
+    for (int k0 = tid; k0 < n_stage; k0 += nth * STG) {
+        double vals[STG];
+#pragma unroll
+        for (int u = 0; u < STG; ++u) {
+            int k = k0 + u * nth;
+            int c = k % UC, rest = k / UC;
+            int r = rest % UR, pl = rest / UR;
+            int ui = iu0 + c, uj = ju0 + r;
+            vals[u] = (k < n_stage && ui >= 0 && ui < nr && uj >= 0 && uj < nt)
+                          ? __ldg(P.u_in + pl * P.plane + (long)uj * P.pitch + ui) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < STG; ++u) {
+            int k = k0 + u * nth;
+            if (k < n_stage) us[k] = vals[u];
+        }
     }
     __syncthreads();
 
@@ -358,13 +371,24 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel_col(StepParams P, Thet
     const int i0 = blockIdx.x * TI, iu0 = i0 - 1;
     const int tid = threadIdx.x, nth = MAXT;
 
-    for (int k = tid; k < 4 * L * nt * UC; k += nth) {
-        int c = k % UC, rest = k / UC;
-        int r = rest % nt, pl = rest / nt;
-        int ui = iu0 + c;
-        double val = 0.0;
-        if (ui >= 0 && ui < nr) val = __ldg(P.u_in + pl * P.plane + (long)r * P.pitch + ui);
-        us[k] = val;
+    // stage the u^n columns; loads in batches of STG before any store (one memory round trip per batch)
+    constexpr int STG = 8;
+    const int n_stage = 4 * L * nt * UC;
+    for (int k0 = tid; k0 < n_stage; k0 += nth * STG) {
+        double vals[STG];
+#pragma unroll
+        for (int u = 0; u < STG; ++u) {
+            int k = k0 + u * nth;
+            int c = k % UC, rest = k / UC;
+            int r = rest % nt, pl = rest / nt;
+            int ui = iu0 + c;
+            vals[u] = (k < n_stage && ui >= 0 && ui < nr) ? __ldg(P.u_in + pl * P.plane + (long)r * P.pitch + ui) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < STG; ++u) {
+            int k = k0 + u * nth;
+            if (k < n_stage) us[k] = vals[u];
+        }
     }
     __syncthreads();
 
