@@ -24,6 +24,7 @@ sys.path.insert(0, ROOT)
 
 ALG_BYTES_PER_UPDATE = {1: 192.0, 2: 384.0, 4: 768.0}     # 4L read + 4L write + 16L coefficients, x 8 B
 FALLBACK_HBM_GBS = 6650.0
+FP64_INST_PER_UPDATE = {2: 1294.0, 4: 13320.0}            # DADD + DMUL + DFMA thread instructions per update, ncu (profiles/)
 
 
 def parse():
@@ -221,8 +222,16 @@ def cpu_baseline(w):
     t0 = time.perf_counter()
     o.step(steps)
     dt = time.perf_counter() - t0
+    # the same sample on ONE host thread (single-core and all-core figures side by side)
+    oracle.set_threads(1)
+    s1 = max(1, steps // 8)
+    t1 = time.perf_counter()
+    o.step(s1)
+    dt1 = time.perf_counter() - t1
+    oracle.set_threads(cores)
     return {"value": n_win * w.n_theta * steps / dt, "unit": "updates/s", "cores": cores, "kind": "oracle",
-            "sample": f"radial window of {n_win} of {w.n_r} columns x {w.n_theta} rows, {steps} steps, {w.name}"}
+            "sample": f"radial window of {n_win} of {w.n_r} columns x {w.n_theta} rows, {steps} steps, {w.name}",
+            "single_core_value": n_win * w.n_theta * s1 / dt1}
 
 
 def load_traffic(name):
@@ -242,7 +251,7 @@ def run_sweep(args):
     torch.cuda.set_device(0)
     peak, _ = measured_peaks()
     pipe = teuk.bench_fp64("dadd")
-    inst = {2: 1294.0, 4: 13320.0}
+    inst = FP64_INST_PER_UPDATE
     for L in ((1, 2, 4) if not args.precisions else [int(x) for x in args.precisions.split(",")]):
         for nr in (4096, 16384, 65536):
             for nt in (32, 64, 256):
@@ -413,9 +422,12 @@ def main():
         for name, k_steps in (("cfg3", max(50, args.steps // 10)), ("cfg4", max(50, args.steps // 10))):
             wx = workload(name)
             msx, lx, gx, fx = time_device(torch, teuk, wx, k_steps, 20, args.option)
+            upsx = wx.n_r * wx.n_theta * k_steps / (msx * 1e-3)
             per[name] = {"precision_limbs": wx.precision, "n_r": wx.n_r, "n_theta": wx.n_theta, "steps": k_steps,
-                         "updates_per_s": wx.n_r * wx.n_theta * k_steps / (msx * 1e-3), "ms_per_step": msx / k_steps,
-                         "geometry": gx, "finite": fx}
+                         "updates_per_s": upsx, "ms_per_step": msx / k_steps, "geometry": gx, "finite": fx,
+                         # FP64 instructions per update from ncu (profiles/r01e_step_kernels_ncu.md) x rate / measured DADD issue peak
+                         "roofline": {"bound": "fp64 pipe", "fp64_inst_per_update": FP64_INST_PER_UPDATE[wx.precision],
+                                      "peak_inst_per_s": fp["dadd"], "frac": upsx * FP64_INST_PER_UPDATE[wx.precision] / fp["dadd"]}}
         # NEXT-1: the same three workloads with the 10th-order theta operator (column kernel)
         t10 = {}
         for name, k_steps in (("cfg2", max(50, args.steps // 10)), ("cfg3", max(50, args.steps // 10)), ("cfg4", max(50, args.steps // 10))):
