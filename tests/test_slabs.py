@@ -1,6 +1,6 @@
 """NEXT-4 (r*-slab decomposition, paper_1006_0663_b200/slabs.py).
 
-CPU: the index logic, and a world_size-2 gloo run whose per-rank stepper is an oracle window - the sharded run with
+CPU: the index logic, and world_size-2 and -3 gloo runs whose per-rank stepper is an oracle window - the sharded run with
 one halo exchange per `exchange_every` iterations must equal the full-grid oracle BIT FOR BIT on every owned column
 (domain of dependence: r* reach of Eqs. 13-14 is one column per iteration).
 GPU (one device, one process, slabs stepped one after another - no ranks waiting on one another): slab handles of the
@@ -99,10 +99,11 @@ def _worker(rank, world, port, out, L, steps, every):
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("L,steps,every", [(1, (40, 7), 16), (2, (21,), 8)])
-def test_two_rank_slab_run_equals_full_grid_oracle_gloo(tmp_path, L, steps, every):
+@pytest.mark.parametrize("world,L,steps,every", [(2, 1, (40, 7), 16), (2, 2, (21,), 8), (3, 1, (25, 6), 8)])
+def test_slab_run_equals_full_grid_oracle_gloo(tmp_path, world, L, steps, every):
+    """world_size 2 and 3 (an interior rank exchanges with both neighbours), fp64 and dd, chunked step calls"""
     out = str(tmp_path / "slab")
-    mp.spawn(_worker, args=(2, _free_port(), out, L, steps, every), nprocs=2, join=True)
+    mp.spawn(_worker, args=(world, _free_port(), out, L, steps, every), nprocs=world, join=True)
     w = _workload()
     u0 = inputs.random_state(w.n_r, w.n_theta, L, seed=5)
     o = oracle.Oracle.from_workload(w, precision=L)
@@ -110,7 +111,7 @@ def test_two_rank_slab_run_equals_full_grid_oracle_gloo(tmp_path, L, steps, ever
     o.step(sum(steps))
     ref = o.read()
     got = np.zeros_like(ref)
-    for r in range(2):
+    for r in range(world):
         d = torch.load(f"{out}.{r}")
         got[..., d["lo"]:d["hi"]] = d["u"].numpy()
         assert d["exchanges"] == sum(-(-n // every) for n in steps)
