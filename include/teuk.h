@@ -120,7 +120,8 @@ const char *teuk_strerror(int code);
  * half != 0), UNFOLDED: b, alpha_R, alpha_I, gamma_R, gamma_I, W_R, W_I, kappa.  Host output. */
 int teuk_get_tables(teuk_ctx *, int half, double *host_out);
 /* FOLDED coefficient planes the step kernel multiplies with, double[8][n_theta][rows], fp64 handles only:
- * coef_variant 0 = the stored planes, 1 = rebuilt from the semi-recompute tables by a kernel. */
+ * coef_variant 0 = the stored planes, 1 = rebuilt from the semi-recompute tables by a kernel, 2 = rebuilt with 1/Sigma
+ * recomputed as well (full recompute). */
 int teuk_get_folded(teuk_ctx *, int half, int coef_variant, double *host_out);
 /* r and r - r_+ at the 2 n_r - 1 integer/half points as quad-double limbs, double[2 n_r - 1][4] each. */
 int teuk_get_radial(teuk_ctx *, double *host_r, double *host_delta);
