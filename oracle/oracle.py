@@ -21,8 +21,8 @@ from . import mp_ref
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle.so")
-_SRC = [os.path.join(_HERE, "teuk_oracle.cpp"), os.path.join(_HERE, "mpx.hpp")]
-CXXFLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared"]
+_SRC = [os.path.join(_HERE, "teuk_oracle.cpp"), os.path.join(_HERE, "mpx.hpp"), os.path.join(_HERE, "mpf.hpp")]
+CXXFLAGS = ["-O2", "-std=c++17", "-mfma", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared"]
 _lib = None
 
 
@@ -42,7 +42,7 @@ def lib():
         dp = C.POINTER(C.c_double)
         _lib.oracle_create.argtypes = [C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
                                        C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, dp, dp, dp, dp, dp, dp,
-                                       C.c_int, dp, dp, C.POINTER(C.c_void_p)]
+                                       C.c_int, dp, dp, C.c_int, C.POINTER(C.c_void_p)]
         _lib.oracle_set_observer.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_long]
         _lib.oracle_set_initial.argtypes = [C.c_void_p, dp, C.c_int]
         _lib.oracle_step.argtypes = [C.c_void_p, C.c_long]
@@ -57,6 +57,9 @@ def lib():
         _lib.oracle_destroy.argtypes = [C.c_void_p]
         _lib.oracle_destroy.restype = None
         _lib.oracle_mp_op.argtypes = [C.c_int, C.c_int, dp, dp, dp]
+        _lib.oracle_mpf_op.argtypes = [C.c_int, C.c_int, dp, dp, dp]
+        _lib.oracle_mp_op_batch.argtypes = [C.c_int, C.c_int, C.c_int, C.c_long, dp, dp, dp]
+        _lib.oracle_set_zero_fast_path.argtypes = [C.c_int]
         _lib.oracle_set_threads.argtypes = [C.c_int]
     return _lib
 
@@ -66,15 +69,35 @@ def _dp(a: np.ndarray):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 
 
-def mp_op(op: str, n: int, a, b=None) -> list:
-    """Test hook (pin P1): one N-limb operation of the oracle's arithmetic."""
-    code = {"add": 0, "sub": 1, "mul": 2, "div": 3, "sqrt": 4, "mul_d": 5}[op]
+_OPS = {"add": 0, "sub": 1, "mul": 2, "div": 3, "sqrt": 4, "mul_d": 5, "half": 6}
+TIERS = {"exact": 0, "fast": 1}
+
+
+def mp_op(op: str, n: int, a, b=None, tier: str = "exact") -> list:
+    """Test hook (pin P1): one N-limb operation of the oracle's arithmetic (tier "exact": mpx.hpp, "fast": mpf.hpp)."""
     aa = np.array(list(a) + [0.0] * (4 - len(a)), dtype=np.float64)
     bb = np.array(list(b if b is not None else [1.0]) + [0.0] * 4, dtype=np.float64)[:4].copy()
     out = np.zeros(4)
-    rc = lib().oracle_mp_op(code, n, _dp(aa), _dp(bb), _dp(out))
+    fn = lib().oracle_mpf_op if TIERS[tier] else lib().oracle_mp_op
+    rc = fn(_OPS[op], n, _dp(aa), _dp(bb), _dp(out))
     assert rc == 0
     return [float(v) for v in out[:n]]
+
+
+def mp_op_batch(op: str, n: int, a: np.ndarray, b: np.ndarray, tier: str = "exact") -> np.ndarray:
+    """The same hook on a corpus: a, b [count][n] -> [count][n]."""
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    assert a.shape == b.shape and a.shape[1] == n
+    out = np.zeros_like(a)
+    rc = lib().oracle_mp_op_batch(TIERS[tier], _OPS[op], n, a.shape[0], _dp(a), _dp(b), _dp(out))
+    assert rc == 0
+    return out
+
+
+def set_zero_fast_path(on: bool) -> bool:
+    """Test hook: switch the x + 0 = x / x * 0 = 0 shortcuts of the fast tier (mpf.hpp); returns the old setting."""
+    return bool(lib().oracle_set_zero_fast_path(int(on)))
 
 
 def set_threads(n: int) -> int:
@@ -88,7 +111,7 @@ class Oracle:
     """Plain CPU solver of PAPER.md §III.B; see teuk_oracle.cpp for the step-by-step citations."""
 
     def __init__(self, M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision, i_lo=0, n_win=None,
-                 theta_order=2):
+                 theta_order=2, tier="exact"):
         self.n_win = n_r - i_lo if n_win is None else n_win
         self.n_r, self.n_theta, self.L, self.i_lo = n_r, n_theta, precision, i_lo
         self.s, self.m = s, m
@@ -102,15 +125,15 @@ class Oracle:
         self.h = C.c_void_p()
         k = [_dp(x) for x in self._keep]
         rc = lib().oracle_create(M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision, i_lo, self.n_win,
-                                 *k[:6], theta_order, k[6], k[7], C.byref(self.h))
+                                 *k[:6], theta_order, k[6], k[7], TIERS[tier], C.byref(self.h))
         if rc != 0:
             self.h = None
             raise ValueError(f"oracle_create failed: {rc}")
 
     @classmethod
-    def from_workload(cls, w, precision=None, i_lo=0, n_win=None, theta_order=2):
+    def from_workload(cls, w, precision=None, i_lo=0, n_win=None, theta_order=2, tier="exact"):
         return cls(w.M, w.a, w.s, w.m, w.n_r, w.n_theta, w.rstar_min, w.rstar_max, w.dt,
-                   precision or w.precision, i_lo, n_win, theta_order)
+                   precision or w.precision, i_lo, n_win, theta_order, tier)
 
     def __del__(self):
         if getattr(self, "h", None):

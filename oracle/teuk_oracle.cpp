@@ -11,7 +11,10 @@
 //   O6  full step, Eq. (14); radial Dirichlet rows.
 //   polar ghosts f_{-1} = sigma f_0, f_{N} = sigma f_{N-1}, sigma = (-1)^{|m|}.
 //   O7  observer at a fixed location, bilinear interpolation (reading A11).
-// T is double, MP<2> (double-double) or MP<4> (quad-double) from mpx.hpp.
+// T is double, MP<2> (double-double) or MP<4> (quad-double) from mpx.hpp (tier 0: every operation exact, then
+// rounded -- the arbitration tier), or FP<2> / FP<4> from mpf.hpp (tier 1: accurate IEEE-style operations, ~20x
+// faster, pinned against tier 0; used for the full-length golden runs of configs 3 and 4).  The stepper below is
+// ONE template: both tiers execute the same statements.  Coefficient tables are always built with MP<4>.
 // A sub-window [i_lo, i_lo+n_win) of the radial grid can be stepped on its own (Dirichlet rows at
 // the window edges, zeroed at set_initial); by the domain of dependence (i-1..i+1 per step) its
 // interior [i_lo+k+1, i_lo+n_win-2-k] equals the full-grid result after k steps.
@@ -23,6 +26,7 @@
 #include <omp.h>
 #endif
 #include "mpx.hpp"
+#include "mpf.hpp"
 
 using namespace orc;
 typedef MP<4> Q;
@@ -75,6 +79,8 @@ template <class T> static inline T half_of(const T& x);
 template <> inline double half_of<double>(const double& x) { return 0.5 * x; }
 template <> inline MP<2> half_of<MP<2>>(const MP<2>& x) { return mul_d(x, 0.5); }
 template <> inline MP<4> half_of<MP<4>>(const MP<4>& x) { return mul_d(x, 0.5); }
+template <> inline FP<2> half_of<FP<2>>(const FP<2>& x) { return half(x); }
+template <> inline FP<4> half_of<FP<4>>(const FP<4>& x) { return half(x); }
 
 struct Base {
     Params P;
@@ -447,20 +453,37 @@ template <int N> static int mp_op_n(int op, const double* a, const double* b, do
     return OK;
 }
 
+// the same hook for the fast tier (mpf.hpp); op 6: half(a)
+template <int N> static int mpf_op_n(int op, const double* a, const double* b, double* out) {
+    FP<N> x = Limbs<FP<N>>::make(a), y = Limbs<FP<N>>::make(b), r;
+    switch (op) {
+        case 0: r = x + y; break;
+        case 1: r = x - y; break;
+        case 2: r = x * y; break;
+        case 5: r = mul_d(x, b[0]); break;
+        case 6: r = half(x); break;
+        default: return EINVAL;
+    }
+    for (int k = 0; k < N; ++k) out[k] = r.x[k];
+    return OK;
+}
+
 // ------------------------------------------------------------------------------------ C ABI
 extern "C" {
 
 int oracle_create(double M, double a, int s, int m, int n_r, int n_theta, double rmin, double rmax, double dt,
                   int precision, int i_lo, int n_win, const double* r_tab, const double* d_tab, const double* sin_tab,
                   const double* cos_tab, const double* dr_l, const double* dth_l, int theta_order, const double* wc_l,
-                  const double* wd_l, void** out) {
+                  const double* wd_l, int tier, void** out) {
     if (!(M > 0) || !(std::fabs(a) < M) || n_r < 3 || n_theta < 2 || !(dt > 0) || !(rmin < rmax) || !out) return EINVAL;
     if ((theta_order != 2 && theta_order != 10) || n_theta < theta_order / 2) return EINVAL;
     if (i_lo < 0 || n_win < 3 || i_lo + n_win > n_r) return EINVAL;
     Base* b = nullptr;
     if (precision == 1) b = new Solver<double>();
-    else if (precision == 2) b = new Solver<MP<2>>();
-    else if (precision == 4) b = new Solver<MP<4>>();
+    else if (precision == 2 && tier == 0) b = new Solver<MP<2>>();
+    else if (precision == 4 && tier == 0) b = new Solver<MP<4>>();
+    else if (precision == 2 && tier == 1) b = new Solver<FP<2>>();
+    else if (precision == 4 && tier == 1) b = new Solver<FP<4>>();
     else return EINVAL;
     b->P = Params{M, a, dt, rmin, rmax, s, m, n_r, n_theta, precision, i_lo, n_win, theta_order};
     int rc = b->build(r_tab, d_tab, sin_tab, cos_tab, dr_l, dth_l, wc_l, wd_l);
@@ -496,5 +519,21 @@ int oracle_mp_op(int op, int N, const double* a, const double* b, double* out) {
     if (N == 4) return mp_op_n<4>(op, a, b, out);
     return EINVAL;
 }
+
+int oracle_mpf_op(int op, int N, const double* a, const double* b, double* out) {
+    if (N == 2) return mpf_op_n<2>(op, a, b, out);
+    if (N == 4) return mpf_op_n<4>(op, a, b, out);
+    return EINVAL;
+}
+// batched form of both hooks for the corpus tests: n operand pairs, rows of N doubles
+int oracle_mp_op_batch(int tier, int op, int N, long n, const double* a, const double* b, double* out) {
+    for (long k = 0; k < n; ++k) {
+        int rc = tier ? oracle_mpf_op(op, N, a + k * N, b + k * N, out + k * N)
+                      : oracle_mp_op(op, N, a + k * N, b + k * N, out + k * N);
+        if (rc != OK) return rc;
+    }
+    return OK;
+}
+int oracle_set_zero_fast_path(int on) { int old = g_zero_fast_path; g_zero_fast_path = on; return old; }
 
 }  // extern "C"

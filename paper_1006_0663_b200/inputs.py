@@ -82,24 +82,33 @@ class Workload:
         return replace(self, **kw)
 
 
-def stable_dt(w: Workload, z_max: float = 0.2) -> float:
-    """Harness time-step rule (reading A15b).  The two-step scheme of Eqs. (13)-(14) advances an
-    undamped oscillator  Phi_tt = -omega^2 Phi  with amplification 1 + (omega dt)^4/8 per step, so the stiffest
-    angular mode near the peak of kappa = Delta/Sigma^2 (omega^2 ~ kappa_max [4/dtheta^2 + (|m|+|s|)^2 /
-    sin^2(dtheta/2)], the second term being the pole potential of (m + s cos)^2/sin^2) grows unless omega dt is
-    small.  Measured with the oracle: config 2 at dt = 0.5 dr* overflows within 1500 steps.  For (s, m) != (0, 0)
-    the harness therefore passes dt = min(0.5 dr*, z_max / omega_max); work per update is unchanged.
-    This is input generation only (fp64 estimate), not part of the method's arithmetic."""
+def stable_dt(w: Workload, z_max: float | None = None) -> float:
+    """Harness time-step rule (reading A15b; pinned by tests/test_oracle_stability.py).  The two-step
+    scheme of Eqs. (13)-(14) advances an undamped oscillator  Phi_tt = -omega^2 Phi  with
+    amplification 1 + (omega dt)^4/8 per step, so for (s, m) != (0, 0) the stiffest angular mode near the peak of
+    kappa = Delta/Sigma^2 (omega^2 ~ kappa_max [4/dtheta^2 + (|m|+|s|)^2 / sin^2(dtheta/2)], the second term being
+    the pole potential of (m + s cos)^2/sin^2) grows without bound at BASELINE's dt = 0.5 dr*: config 2 gains
+    e^0.125 per step there.  The harness passes dt = min(0.5 dr*, z / omega_max) with
+        z = (8 / N_steps)^(1/4),
+    i.e. the time step for which the scheme's own amplification of the stiffest mode over the WHOLE run,
+    (1 + z^4/8)^N_steps, is at most e (config 2/3: z = 0.141, dt = 0.068 dr*; config 5, 1000 steps: z = 0.299).
+    Work per update is unchanged.  Input generation only (fp64 estimate), not part of the method's arithmetic."""
     half_dr = 0.5 * w.dr
     if w.s == 0 and w.m == 0:
         return half_dr
+    z = z_max if z_max is not None else (8.0 / max(w.steps, 1)) ** 0.25
+    return min(half_dr, z / omega_max(w))
+
+
+def omega_max(w: Workload) -> float:
+    """fp64 estimate of the stiffest angular frequency of the pole rows (see `stable_dt`)."""
     rp = w.M + math.sqrt(w.M * w.M - w.a * w.a)
     r = rp + np.linspace(1e-3, 20.0, 20001)
     delta = r * r - 2.0 * w.M * r + w.a * w.a
     kappa_max = float(np.max(delta / (r * r + w.a * w.a) ** 2))
     dth = math.pi / w.n_theta
     om2 = kappa_max * (4.0 / dth ** 2 + (abs(w.m) + abs(w.s)) ** 2 / math.sin(0.5 * dth) ** 2)
-    return min(half_dr, z_max / math.sqrt(om2))
+    return math.sqrt(om2)
 
 
 def config(k: int) -> Workload:
@@ -121,10 +130,10 @@ def config(k: int) -> Workload:
 
 def sweep_cell(n_r: int, n_theta: int, precision: int) -> Workload:
     """BASELINE.json config 5: a = 0.99, s = -2, m = 2, r* in [-300, 700] (A15), 1000 steps,
-    dt from `stable_dt` (z_max = 0.4: 1000 steps tolerate a larger per-step growth)."""
+    dt from `stable_dt` (z = (8/1000)^(1/4) = 0.299)."""
     w = Workload(f"cfg5_{n_r}x{n_theta}_L{precision}", 1.0, 0.99, -2, 2, n_r, n_theta, -300.0, 700.0,
                  1000, precision, "Y22m2", (100.0, 5.0), (6.0, 1.0), (1.0, 0.0), SEED_BASE + 5)
-    return replace(w, dt_override=stable_dt(w, z_max=0.4))
+    return replace(w, dt_override=stable_dt(w))
 
 
 def theta_profile(profile: str, n_theta: int) -> np.ndarray:
