@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 SO = os.path.join(HERE, "libteuk.so")
-SOURCES = ["teuk.cu", "k_generic1.cu", "k_generic2.cu", "k_generic4.cu", "k_tma.cu", "k_tb2.cu"]
+SOURCES = ["teuk.cu", "k_generic1.cu", "k_generic2.cu", "k_generic4.cu", "k_tma.cu", "k_tb2.cu", "k_march.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=true",
               "-Xcompiler", "-fPIC,-O2,-ffp-contract=off"]
 

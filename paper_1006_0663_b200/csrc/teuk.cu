@@ -8,6 +8,7 @@
 #include <cstdlib>
 #include <algorithm>
 #include <cstring>
+#include <map>
 #include <vector>
 
 #include "../../include/teuk.h"
@@ -17,6 +18,7 @@
 #include "step_kernel.cuh"
 #include "step_kernel_tma.cuh"
 #include "step_kernel_tb2.cuh"
+#include "step_kernel_march.cuh"
 #include "kernels.h"
 
 using namespace tk;
@@ -86,7 +88,9 @@ struct teuk_ctx {
     int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0, theta_order = 2, opt_pdl = 0, opt_tb = 1;   // PDL measured neutral on cfg 2 (40.2 vs 40.0 us): kept as an option
     ThetaWeights tw;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
-    bool use_tma = false, use_rc = false, use_col_tma = false;
+    bool use_tma = false, use_rc = false, use_col_tma = false, use_march = false;
+    int opt_march = 1, march_regs = 0;     // fp64 semi-recompute supply: column-march kernel (step_kernel_march.cuh) unless march=0
+    long march_rows_per_warp = 0, march_total_rows = 0;
     CUtensorMap tm_state[2], tm_ch, tm_ci, tm_ish, tm_isi, tm_rth, tm_rti;
     // temporally blocked fp64 path (two iterations per launch, step_kernel_tb2.cuh): its own boxes, grid and smem
     bool use_tb2 = false;
@@ -111,7 +115,15 @@ struct teuk_ctx {
     long mp_cap = 0;
     int mp_n = 0, mp_i = 0;
     R4 mp_wr;
-    cudaGraphExec_t graph[2] = {nullptr, nullptr};
+    // CUDA graphs of n consecutive iterations starting from state buffer `parity`, keyed by n: n = graph_steps for the
+    // bulk of a teuk_step call and one more entry per distinct remainder (so a 20-iteration call is one graph launch too)
+    std::map<long, cudaGraphExec_t> graph[2];
+    void drop_graphs() {
+        for (int p = 0; p < 2; ++p) {
+            for (auto& kv : graph[p]) cudaGraphExecDestroy(kv.second);
+            graph[p].clear();
+        }
+    }
 
     double* dptr(size_t off) const { return (double*)(ws + off); }
     double* state(int which) const { return dptr(which ? lay.state_b : lay.state_a); }
@@ -395,6 +407,10 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     } else if (!strcmp(key, "time_block")) {
         if ((v != 1 && v != 2) || (v == 2 && c->L != 1)) return TEUK_EINVAL;
         c->opt_tb = v;
+    } else if (!strcmp(key, "march")) {
+        c->opt_march = v != 0;
+    } else if (!strcmp(key, "march_regs")) {
+        c->march_regs = v != 0;
     } else if (!strcmp(key, "use_tma")) {
         c->opt_tma = v != 0;
     } else {
@@ -416,8 +432,7 @@ extern "C" int teuk_set_observer(teuk_ctx* c, double rstar_obs, double theta_obs
     c->wt = sub(y, from_double<4>((double)j0));
     c->oi = i0; c->oj = j0; c->obs_cap = capacity;
     c->nonfinite = false;
-    for (int p = 0; p < 2; ++p)
-        if (c->graph[p]) { cudaGraphExecDestroy(c->graph[p]); c->graph[p] = nullptr; }
+    c->drop_graphs();
     CK(cudaMemsetAsync(c->step_base(), 0, 32, c->stream));
     c->series_origin = c->steps_done;      // both series (point observer and multipoles) restart here
     return TEUK_OK;
@@ -580,6 +595,30 @@ static int choose_geometry(teuk_ctx* c) {
         const void* fn = col_fn(c, &c->threads);
         return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
     }
+    c->use_march = false;
+    if (c->L == 1 && c->coef_variant == 1 && c->opt_march) {
+        // persistent grid: every resident warp gets an equal contiguous share of the strip-rows (strip-major)
+        const void* fn = march_step_fn(c->march_regs);
+        const size_t sm = ((size_t)4 * c->n_theta + (size_t)MARCH_WARPS * 2 * MARCH_NRT * 32) * sizeof(double);
+        int dev = 0, sms = 0, per_sm = 0;
+        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess ||
+            cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * MARCH_WARPS, sm) != cudaSuccess || per_sm < 1)
+            return TEUK_ECUDA;
+        const long strips = (c->n_r + MARCH_W - 1) / MARCH_W;
+        const long total = strips * c->n_theta;
+        const long capacity = (long)sms * per_sm * MARCH_WARPS;
+        long share = (total + capacity - 1) / capacity;
+        const long min_share = std::min(8, c->n_theta);            // below this the two-row theta halo dominates
+        if (share < min_share) share = min_share;
+        const long warps = (total + share - 1) / share;
+        c->march_rows_per_warp = share; c->march_total_rows = total;
+        c->ti = MARCH_W; c->tj = (int)std::min<long>(share, c->n_theta); c->smem = sm; c->threads = 32 * MARCH_WARPS;
+        c->grid = dim3((unsigned)((warps + MARCH_WARPS - 1) / MARCH_WARPS), 1);
+        c->use_march = true;
+        return TEUK_OK;
+    }
     if (c->L == 1 && c->coef_variant >= 1) {
         bool ok = (c->opt_tj == 8) ? setup_rc<32, 8>(c) : setup_rc<32, 16>(c);
         cudaGetLastError();
@@ -648,6 +687,17 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         int threads = 256;
         const void* fn = col_fn(c, &threads);
         if (cudaLaunchKernel(fn, c->grid, dim3(threads), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
+    } else if (c->use_march) {
+        MarchParams Q;
+        Q.isig_i = c->dptr(c->lay.rc_isig);
+        Q.isig_h = c->dptr(c->lay.rc_isig) + c->lay.plane;
+        Q.rt = c->dptr(c->lay.rc_rt);
+        Q.th = c->dptr(c->lay.rc_th);
+        Q.rows_per_warp = c->march_rows_per_warp;
+        Q.total_rows = c->march_total_rows;
+        void* args[] = {&P, &Q};
+        if (cudaLaunchKernel(march_step_fn(c->march_regs), c->grid, dim3(c->threads), args, c->smem, c->stream) != cudaSuccess)
+            return TEUK_ECUDA;
     } else if (c->use_rc || c->use_tma) {
         // programmatic dependent launch: the next step's blocks may start (and prefetch their coefficient tiles) while this
         // step drains; they execute griddepcontrol.wait before touching the state
@@ -750,19 +800,31 @@ extern "C" int teuk_set_initial(teuk_ctx* c, const double* host_planes, int limb
     return TEUK_OK;
 }
 
-static int build_graph(teuk_ctx* c, int parity) {
+// launches n iterations starting from state(from) on the stream (captured or not); *flips = number of buffer swaps,
+// *nl = step-kernel launches.  Sample offsets are relative to the device-side counter, which the trailing
+// advance_kernel moves on by n.
+static int launch_iterations(teuk_ctx* c, int from, long n, int* flips, long* nl) {
+    long k = 0;
+    *flips = 0; *nl = 0;
+    while (k < n) {
+        int rc;
+        if (tb2_active(c) && k + 2 <= n) { rc = launch_step2(c, from, (int)k); k += 2; }
+        else { rc = launch_step(c, from, (int)k); k += 1; }
+        if (rc != TEUK_OK) return rc;
+        from ^= 1; ++*flips; ++*nl;
+    }
+    advance_kernel<<<1, 1, 0, c->stream>>>(c->step_base(), n);
+    return cudaGetLastError() == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
+}
+
+static int build_graph(teuk_ctx* c, int parity, long n, cudaGraphExec_t* out) {
     cudaGraph_t g;
     CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
-    int from = parity, rc = TEUK_OK;
-    const int stride = tb2_active(c) ? 2 : 1;       // graph_steps is even
-    for (int k = 0; k < c->graph_steps && rc == TEUK_OK; k += stride) {
-        rc = stride == 2 ? launch_step2(c, from, k) : launch_step(c, from, k);
-        from ^= 1;
-    }
-    advance_kernel<<<1, 1, 0, c->stream>>>(c->step_base(), c->graph_steps);
+    int flips; long nl;
+    int rc = launch_iterations(c, parity, n, &flips, &nl);
     cudaError_t e = cudaStreamEndCapture(c->stream, &g);
     if (rc != TEUK_OK || e != cudaSuccess) return TEUK_ECUDA;
-    e = cudaGraphInstantiate(&c->graph[parity], g, 0);
+    e = cudaGraphInstantiate(out, g, 0);
     cudaGraphDestroy(g);
     return e == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
 }
@@ -772,36 +834,29 @@ extern "C" int teuk_step(teuk_ctx* c, long n) {
     if (!c->have_init) return TEUK_ESTATE;
     long left = n;
     // the legacy default stream cannot be captured: plain launches there
-    const int K = (c->stream == nullptr || c->stream == cudaStreamLegacy) ? 0 : c->graph_steps;
-    while (K > 0 && left >= K) {
-        if (!c->graph[c->cur]) {
-            int rc = build_graph(c, c->cur);
-            if (rc != TEUK_OK) return rc;
-        }
-        CK(cudaGraphLaunch(c->graph[c->cur], c->stream));
-        if (tb2_active(c)) {
-            c->launches += K / 2 + 1;
-            c->cur ^= (K / 2) & 1;            // one buffer flip per two-iteration launch
+    const long K = (c->stream == nullptr || c->stream == cudaStreamLegacy) ? 0 : c->graph_steps;
+    while (left > 0) {
+        const long chunk = (K > 0 && left >= K) ? K : left;
+        // launches and buffer swaps of a chunk (a two-iteration launch swaps once)
+        const long nl = tb2_active(c) ? chunk / 2 + (chunk & 1) : chunk;
+        const bool graphable = K > 0 && chunk >= 2 && (chunk == K || c->graph[c->cur].size() < 16);
+        if (graphable) {
+            auto it = c->graph[c->cur].find(chunk);
+            if (it == c->graph[c->cur].end()) {
+                cudaGraphExec_t ge = nullptr;
+                int rc = build_graph(c, c->cur, chunk, &ge);
+                if (rc != TEUK_OK) return rc;
+                it = c->graph[c->cur].emplace(chunk, ge).first;
+            }
+            CK(cudaGraphLaunch(it->second, c->stream));
         } else {
-            c->launches += (c->mp_cap > 0 ? 2 * K : K) + 1;      // K is even: c->cur unchanged
-        }
-        left -= K;
-    }
-    if (left > 0) {
-        long k = 0, nl = 0;
-        for (; tb2_active(c) && k + 2 <= left; k += 2, ++nl) {
-            int rc = launch_step2(c, c->cur, (int)k);
+            int flips; long nl2;
+            int rc = launch_iterations(c, c->cur, chunk, &flips, &nl2);
             if (rc != TEUK_OK) return rc;
-            c->cur ^= 1;
         }
-        for (; k < left; ++k, ++nl) {
-            int rc = launch_step(c, c->cur, (int)k);
-            if (rc != TEUK_OK) return rc;
-            c->cur ^= 1;
-        }
-        advance_kernel<<<1, 1, 0, c->stream>>>(c->step_base(), left);
+        c->cur ^= (int)(nl & 1);
         c->launches += (c->mp_cap > 0 ? 2 * nl : nl) + 1;
-        if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
+        left -= chunk;
     }
     c->steps_done += n;
     return TEUK_OK;
@@ -966,8 +1021,7 @@ extern "C" int teuk_set_multipole_observer(teuk_ctx* c, double rstar_obs, int n_
             for (int l = 0; l < L; ++l) q[((size_t)k * L + l) * nt + j] = w.x[l];
         }
     }
-    for (int p = 0; p < 2; ++p)
-        if (c->graph[p]) { cudaGraphExecDestroy(c->graph[p]); c->graph[p] = nullptr; }
+    c->drop_graphs();
     CK(cudaMemcpyAsync(c->dptr(c->lay.mp_q), q.data(), q.size() * 8, cudaMemcpyHostToDevice, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return TEUK_OK;
@@ -1005,8 +1059,8 @@ extern "C" int teuk_step_geometry(teuk_ctx* c, long* o) {
 }
 extern "C" void teuk_destroy(teuk_ctx* c) {
     if (!c) return;
-    for (int p = 0; p < 2; ++p)
-        if (c->graph[p]) cudaGraphExecDestroy(c->graph[p]);
+    cudaStreamSynchronize(c->stream);      // the caller may recycle the workspace as soon as this returns
+    c->drop_graphs();
     delete c;
 }
 extern "C" const char* teuk_strerror(int code) {
