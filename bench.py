@@ -22,9 +22,20 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-ALG_BYTES_PER_UPDATE = {1: 192.0, 2: 384.0, 4: 768.0}     # 4L read + 4L write + 16L coefficients, x 8 B
+ALG_BYTES_PER_UPDATE = {1: 192.0, 2: 384.0, 4: 768.0}     # DESIGN.md §6, stored planes: 4L read + 4L write + 16L coefficients, x 8 B
+SEMI_RECOMPUTE_BYTES = 80.0                               # fp64 semi-recompute supply: 64 B of state + two 1/Sigma values
 FALLBACK_HBM_GBS = 6650.0
-FP64_INST_PER_UPDATE = {2: 1294.0, 4: 13320.0}            # DADD + DMUL + DFMA thread instructions per update, ncu (profiles/)
+REPS = 5                                                  # timed repetitions of the K-step region; median and min are reported
+DTYPE = {1: "f64", 2: "f64x2 (double-double)", 4: "f64x4 (quad-double)"}
+
+
+def fp64_inst_per_update():
+    """FP64 (DADD + DMUL + DFMA) thread instructions per update of the dd / qd step kernels: `measured` = ncu count of the
+    kernel as built (redundant halo half steps included), `method` = the count of the update itself (no halo work).
+    Written next to the ncu summary it comes from (profiles/fp64_inst.json names the capture and the csrc/ revision)."""
+    with open(os.path.join(ROOT, "profiles", "fp64_inst.json")) as f:
+        d = json.load(f)
+    return {(2, 2): d["dd"], (4, 2): d["qd"], (2, 10): d["dd_theta10"], (4, 10): d["qd_theta10"]}
 
 
 def parse():
@@ -128,12 +139,11 @@ def run_reference(args):
     n_win = min(w.n_r, 2048)
     i_lo = max(0, int((inputs.pulse_parameters(w)[0] - w.rstar_min) / w.dr) - n_win // 2)
     cores = oracle.set_threads(0)
-    o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win)
+    o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win, tier="exact" if w.precision == 1 else "fast")
     u0 = inputs.initial_state(w)[..., i_lo:i_lo + n_win]
     o.set_initial(np.ascontiguousarray(u0))
-    per = {1: 1, 2: 1, 4: 1}[w.precision]
-    o.step(args.warmup * per if w.precision == 1 else min(args.warmup, 2))
-    steps = args.steps if w.precision == 1 else max(1, min(args.steps, 20))
+    o.step(args.warmup if w.precision == 1 else min(args.warmup, 2))
+    steps = args.steps if w.precision == 1 else max(1, min(args.steps, 40))
     t0 = time.perf_counter()
     o.step(steps)
     dt = time.perf_counter() - t0
@@ -142,8 +152,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": "Teukolsky grid-point updates/s", "value": val, "unit": "updates/s",
             "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": {1: "f64", 2: "f64x2 (double-double)", 4: "f64x4 (quad-double)"}[w.precision],
-            "data": "synthetic", "config": {"workload": w.name, "n_r": w.n_r, "n_theta": w.n_theta, "sample": sample},
+            "dtype": DTYPE[w.precision],
+            "data": "synthetic", "config": {"workload": w.name, "n_r": w.n_r, "n_theta": w.n_theta,
+                                            "dt_over_dr": w.dt / w.dr, "sample": sample},
             "cpu_baseline": {"value": val, "unit": "updates/s", "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": "updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -160,31 +171,50 @@ def make_solver(teuk, w, options, obs_capacity):
     return g
 
 
-def time_device(torch, teuk, w, steps, warmup, options, dist=None):
-    """inputs resident in HBM; CUDA events on the stream the kernels are launched on."""
+_flush_buf = None
+
+
+def flush_l2(torch, device):
+    """write a buffer larger than the 126 MB L2 (between timed repetitions)"""
+    global _flush_buf
+    if _flush_buf is None or _flush_buf.device != torch.device(device):
+        _flush_buf = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=device)
+    _flush_buf.fill_(1)
+
+
+def time_device(torch, teuk, w, steps, warmup, options, dist=None, reps=REPS):
+    """inputs resident in HBM; CUDA events on the stream the kernels are launched on.  W untimed warm-up iterations and one
+    untimed K-iteration call (which instantiates the CUDA graph of that call), then REPS timed repetitions of exactly K
+    iterations each, L2 flushed between repetitions.  Returns the median repetition (ms) and the rest beside it."""
     from paper_1006_0663_b200 import inputs
-    g = make_solver(teuk, w, options, warmup + steps)
+    g = make_solver(teuk, w, options, warmup + steps * (reps + 1))
     u0 = torch.from_numpy(inputs.initial_state(w)).to(g.device)
     g.set_initial(u0)
     g.step(warmup)
-    torch.cuda.synchronize()
-    if dist is not None:
-        dist.barrier()
-    n0 = g.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(g.stream)
     g.step(steps)
-    e1.record(g.stream)
     torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1)
-    if dist is not None:
-        dist.barrier()
-    launches = g.launch_count() - n0
+    times, launches = [], 0
+    for _ in range(reps):
+        flush_l2(torch, g.device)
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        n0 = g.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(g.stream)
+        g.step(steps)
+        e1.record(g.stream)
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1))
+        if dist is not None:
+            dist.barrier()
+        launches = g.launch_count() - n0
     geom = g.step_geometry()
-    ser = g.observe(4, allow_nonfinite=True)
+    g.observe(4, allow_nonfinite=True)
     finite = bool(torch.isfinite(g.read_device()).all().item()) and g.last_observe_status == 0
     g.close()
-    return ms, launches, geom, finite
+    ts = sorted(times)
+    return {"ms": ts[len(ts) // 2], "ms_min": ts[0], "ms_all": times, "launches": launches, "geometry": geom, "finite": finite}
 
 
 def time_e2e(torch, teuk, w, steps, options):
@@ -208,17 +238,23 @@ def time_e2e(torch, teuk, w, steps, options):
 
 
 def cpu_baseline(w):
-    """the oracle as it stands, on this box's host cores, on a bounded sample of the same workload."""
+    """the oracle as it stands, on this box's host cores, on a bounded sample of the same workload (fp64: the plain
+    double stepper; dd/qd: its fast arithmetic tier, the one the full-length golden runs use)."""
     import numpy as np
     from oracle import oracle
     from paper_1006_0663_b200 import inputs
     n_win = min(w.n_r, 1024)
     i_lo = max(0, int((inputs.pulse_parameters(w)[0] - w.rstar_min) / w.dr) - n_win // 2)
     cores = oracle.set_threads(0)
-    o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win)
+    tier = "exact" if w.precision == 1 else "fast"
+    o = oracle.Oracle.from_workload(w, i_lo=i_lo, n_win=n_win, tier=tier)
     o.set_initial(np.ascontiguousarray(inputs.initial_state(w)[..., i_lo:i_lo + n_win]))
-    steps = {1: 400, 2: 8, 4: 4}[w.precision]
     o.step(2)
+    # size the sample for a few seconds of CPU work from a short probe
+    t0 = time.perf_counter()
+    o.step(2)
+    probe = (time.perf_counter() - t0) / 2
+    steps = int(max(4, min(2000, 5.0 / max(probe, 1e-6))))
     t0 = time.perf_counter()
     o.step(steps)
     dt = time.perf_counter() - t0
@@ -229,7 +265,7 @@ def cpu_baseline(w):
     o.step(s1)
     dt1 = time.perf_counter() - t1
     oracle.set_threads(cores)
-    return {"value": n_win * w.n_theta * steps / dt, "unit": "updates/s", "cores": cores, "kind": "oracle",
+    return {"value": n_win * w.n_theta * steps / dt, "unit": "updates/s", "cores": cores, "kind": "oracle", "tier": tier,
             "sample": f"radial window of {n_win} of {w.n_r} columns x {w.n_theta} rows, {steps} steps, {w.name}",
             "single_core_value": n_win * w.n_theta * s1 / dt1}
 
@@ -242,35 +278,72 @@ def load_traffic(name):
         return None
 
 
+def supply_of(options, L):
+    """(label, algorithmic bytes per update) of the coefficient supply the option list selects"""
+    opt = {o.replace(" ", "") for o in options}
+    if L == 1 and "coef_variant=1" in opt:
+        return "semi_recompute", SEMI_RECOMPUTE_BYTES
+    if L == 1 and "coef_variant=2" in opt:
+        return "full_recompute", 64.0
+    if L == 1 and "time_block=2" in opt:
+        return "stored_planes_time_block_2", 96.0
+    return "stored_planes", ALG_BYTES_PER_UPDATE[L]
+
+
+def hbm_roofline(ups, points, bytes_per_update, peak, peak_src, kernel, traffic=None):
+    achieved = ups * bytes_per_update / 1e9
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+            "peak_source": peak_src, "kernel": kernel, "algorithmic_bytes_per_update": bytes_per_update,
+            "algorithmic_bytes_per_launch": bytes_per_update * points}
+
+
+def pipe_roofline(ups, L, pipe_peak, theta_order=2):
+    inst = fp64_inst_per_update()[(L, theta_order)]
+    return {"bound": "alu", "pipe": "fp64", "achieved": ups * inst["measured"], "peak": pipe_peak, "unit": "FP64 inst/s",
+            "frac": ups * inst["measured"] / pipe_peak, "frac_method_only": ups * inst["method"] / pipe_peak,
+            "fp64_inst_per_update_measured": inst["measured"], "fp64_inst_per_update_method": inst["method"],
+            "inst_source": inst.get("source"), "peak_source": "teuk_bench_fp64 DADD chains, this run", "traffic": None}
+
+
+def kernel_name(L, options):
+    opt = {o.replace(" ", "") for o in options}
+    if "theta_order=10" in opt:
+        return "step_kernel_f64_col_tma" if L == 1 else f"step_kernel_col<{L}>"
+    if L == 1:
+        if "coef_variant=1" in opt:
+            return "step_kernel_f64_rc" if "march=0" in opt else "step_kernel_f64_march"
+        if "coef_variant=2" in opt:
+            return "step_kernel_f64_rc<full>"
+        return "step2_kernel_f64_tma" if "time_block=2" in opt else "step_kernel_f64_tma"
+    return f"step_kernel<{L}>"
+
+
 def run_sweep(args):
-    """BASELINE.json config 5 (a = 0.99, s = -2, m = 2): updates/s and roofline fraction per cell.  fp64: HBM fraction
-    (192 B/update vs MEASURED_PEAKS hbm_gbs); dd/qd: FP64-pipe fraction = measured FP64 thread instructions per update
-    (ncu, profiles/r01b_step_kernels_ncu.md: 1294 dd, 13320 qd FP64 instructions per update (profiles/r01c_dd_qd_ncu.md), redundant halo work included) x updates/s / measured DFMA-chain peak."""
+    """BASELINE.json config 5 (a = 0.99, s = -2, m = 2): updates/s and roofline fraction per cell.  fp64: HBM fraction of
+    the selected coefficient supply; dd/qd: FP64-pipe fraction = FP64 thread instructions per update (profiles/fp64_inst.json)
+    x updates/s / DADD issue rate measured in this run."""
     import torch
     from paper_1006_0663_b200 import teuk
     torch.cuda.set_device(0)
-    peak, _ = measured_peaks()
+    peak, peak_src = measured_peaks()
     pipe = teuk.bench_fp64("dadd")
-    inst = FP64_INST_PER_UPDATE
     for L in ((1, 2, 4) if not args.precisions else [int(x) for x in args.precisions.split(",")]):
         for nr in (4096, 16384, 65536):
             for nt in (32, 64, 256):
                 w = workload(f"sweep:{nr}x{nt}:{L}")
-                steps = {1: 1000, 2: 300, 4: 100}[L] if args.steps == 2000 else args.steps
-                ms, launches, geom, finite = time_device(torch, teuk, w, steps, 10, args.option)
-                ups = nr * nt * steps / (ms * 1e-3)
+                steps = {1: 400, 2: 120, 4: 40}[L] if args.steps == 2000 else args.steps
+                r = time_device(torch, teuk, w, steps, 10, args.option, reps=3)
+                ups = nr * nt * steps / (r["ms"] * 1e-3)
+                label, bpu = supply_of(args.option, L)
                 line = {"workload": w.name, "precision_limbs": L, "n_r": nr, "n_theta": nt, "steps": steps,
-                        "dt_over_dr": w.dt / w.dr, "updates_per_s": ups, "ms_per_step": ms / steps, "finite": finite,
-                        "geometry": geom}
+                        "dt_over_dr": w.dt / w.dr, "updates_per_s": ups, "ms_per_step": r["ms"] / steps,
+                        "ms_per_step_min": r["ms_min"] / steps, "finite": r["finite"], "geometry": r["geometry"],
+                        "supply": label}
                 if L == 1:
-                    opt = [o.replace(" ", "") for o in args.option]
-                    bpu = 80.0 if "coef_variant=1" in opt else 64.0 if "coef_variant=2" in opt else 96.0 if "time_block=2" in opt else 192.0
-                    line["roofline"] = {"bound": "hbm", "frac": ups * bpu / 1e9 / peak, "peak_gbs": peak,
-                                        "algorithmic_bytes_per_update": bpu,
-                                        "working_set_mib": 24 * nr * nt * 8 // 2 ** 20}
+                    line["roofline"] = hbm_roofline(ups, nr * nt, bpu, peak, peak_src, kernel_name(L, args.option))
+                    line["working_set_mib"] = int((bpu + 64) * nr * nt) // 2 ** 20
                 else:
-                    line["roofline"] = {"bound": "fp64 pipe", "frac": ups * inst[L] / pipe, "peak_inst_per_s": pipe,
-                                        "fp64_inst_per_update": inst[L]}
+                    line["roofline"] = pipe_roofline(ups, L, pipe, 10 if "theta_order=10" in args.option else 2)
                 print(json.dumps(line), flush=True)
 
 
@@ -332,11 +405,11 @@ def run_slabs(args):
     if rank == 0:
         peak, peak_src = measured_peaks()
         L = w.precision
-        ach = ALG_BYTES_PER_UPDATE[L] * (slab.n_win * w.n_theta) / (ms / args.steps * 1e-3) / 1e9
+        ach = supply_of(args.option, L)[1] * (slab.n_win * w.n_theta) / (ms / args.steps * 1e-3) / 1e9
         print(json.dumps({
             "metric": "Teukolsky grid-point updates/s", "value": value, "unit": "updates/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
-            "scaling": "strong", "vs_baseline": None, "dtype": {1: "f64", 2: "f64x2 (double-double)", 4: "f64x4 (quad-double)"}[L],
+            "scaling": "strong", "vs_baseline": None, "dtype": DTYPE[L],
             "data": "synthetic",
             "config": {"workload": w.name, "n_r": w.n_r, "n_theta": w.n_theta, "precision_limbs": L,
                        "parallelism": f"r*-slabs x{world}, halo {slab.halo}, one exchange per {every} iterations",
@@ -351,6 +424,35 @@ def run_slabs(args):
                          "note": "rank 0's window incl. halo columns"}}), flush=True)
     if d is not None:
         d.destroy_process_group()
+
+
+def measure(torch, teuk, name, steps, warmup, options, peak, peak_src, pipe, dist=None, with_cpu=True, with_e2e=True):
+    """one workload: device-timed rate (median of REPS), roofline of its step kernel, e2e through host buffers, oracle beside it"""
+    w = workload(name) if isinstance(name, str) else name
+    L, points = w.precision, w.n_r * w.n_theta
+    r = time_device(torch, teuk, w, steps, warmup, options, dist)
+    ups = points * steps / (r["ms"] * 1e-3)
+    label, bpu = supply_of(options, L)
+    out = {"workload": w.name, "precision_limbs": L, "dtype": DTYPE[L], "n_r": w.n_r, "n_theta": w.n_theta,
+           "dt_over_dr": w.dt / w.dr, "baseline_dt_over_dr": 0.5, "steps": steps, "updates_per_s": ups,
+           "ms_per_step": r["ms"] / steps, "ms_per_step_min": r["ms_min"] / steps,
+           "ms_per_step_all": [t / steps for t in r["ms_all"]], "gpu_launches": r["launches"], "geometry": r["geometry"],
+           "finite": r["finite"], "coefficient_supply": label}
+    kern = kernel_name(L, options)
+    if L == 1:
+        out["roofline"] = hbm_roofline(ups, points, bpu, peak, peak_src, kern, load_traffic(f"{w.name}:{kern}"))
+        out["working_set_mib"] = int((bpu + 64) * points) // 2 ** 20
+    else:
+        out["roofline"] = pipe_roofline(ups, L, pipe, 10 if "theta_order=10" in options else 2)
+        out["roofline"]["kernel"] = kern
+        out["hbm_frac_at_this_rate"] = ups * ALG_BYTES_PER_UPDATE[L] / 1e9 / peak
+    if with_e2e:
+        dt, h2d, d2h = time_e2e(torch, teuk, w, steps, options)
+        out["e2e"] = {"value": points * steps / dt, "unit": "updates/s", "h2d_bytes_per_step": h2d / steps,
+                      "d2h_bytes_per_step": d2h / steps}
+    if with_cpu:
+        out["cpu_baseline"] = cpu_baseline(w)
+    return out, r
 
 
 def main():
@@ -372,91 +474,84 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         d = dist
-    from paper_1006_0663_b200 import teuk
+    from paper_1006_0663_b200 import replicas, teuk
     w = workload(args.workload)
     L = w.precision
     points = w.n_r * w.n_theta
+    # headline path for fp64: the semi-recompute coefficient supply (H1b variant (b), 80 B/update) unless the caller chose
+    # a supply; dd/qd: stored planes (they are FP64-pipe bound)
+    opts = list(args.option)
+    chose = any(o.replace(" ", "").split("=")[0] in ("coef_variant", "time_block", "use_tma", "theta_order") for o in opts)
+    if L == 1 and not chose:
+        opts.append("coef_variant=1")
+    other = [o for o in opts if not o.replace(" ", "").startswith("coef_variant")]
+    peak, peak_src = measured_peaks()
+    pipe = teuk.bench_fp64("dadd")
+    extra = not args.no_extra and world == 1
     with ClockSampler(local) as cs:
-        ms, launches, geom, finite = time_device(torch, teuk, w, args.steps, args.warmup, args.option, d)
+        head, r = measure(torch, teuk, w, args.steps, args.warmup, opts, peak, peak_src, pipe, d,
+                          with_cpu=extra and rank == 0, with_e2e=False)
     clocks = cs.summary()
-    from paper_1006_0663_b200 import replicas
     # max over ranks of the device time, updates summed over ranks; replicas only, no data-path collective
-    ms_max, _, value = replicas.aggregate(ms, float(points) * args.steps, d, device="cuda")
-    e2e_dt, h2d, d2h = time_e2e(torch, teuk, w, args.steps, args.option)
+    ms_max, _, value = replicas.aggregate(r["ms"], float(points) * args.steps, d, device="cuda")
+    e2e_dt, h2d, d2h = time_e2e(torch, teuk, w, args.steps, opts)
     _, _, e2e_val = replicas.aggregate(e2e_dt * 1e3, float(points) * args.steps, d, device="cuda")
     if rank != 0:
         if d is not None:
             d.destroy_process_group()
         return
-    peak, peak_src = measured_peaks()
-    opt_set = {o.replace(" ", "") for o in args.option}
-    recompute = "coef_variant=1" in opt_set or "coef_variant=2" in opt_set
-    # H1b variant (b): state 64 B + two 1/Sigma planes 16 B; (c): state only; NEXT-3: half of the stored-plane traffic
-    bytes_per_update = (80.0 if "coef_variant=1" in opt_set else 64.0 if "coef_variant=2" in opt_set
-                        else 96.0 if "time_block=2" in opt_set and L == 1 else ALG_BYTES_PER_UPDATE[L])
-    alg_bytes = bytes_per_update * points
-    achieved = alg_bytes / (ms / args.steps * 1e-3) / 1e9
+    label, bpu = supply_of(opts, L)
+    ws_mib = int(((bpu + 64) if L == 1 else 24 * 8 * L) * points) // 2 ** 20
     line = {
         "metric": "Teukolsky grid-point updates/s", "value": value, "unit": "updates/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None,
-        "dtype": {1: "f64", 2: "f64x2 (double-double)", 4: "f64x4 (quad-double)"}[L], "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": DTYPE[L], "data": "synthetic",
         "config": {"workload": w.name, "M": w.M, "a": w.a, "s": w.s, "m": w.m, "n_r": w.n_r, "n_theta": w.n_theta,
-                   "dt_over_dr": w.dt / w.dr, "precision_limbs": L, "parallelism": f"replicas x{world}",
-                   "l2": "working set (2 state copies + 16L coefficient planes = %d MiB) exceeds the 126 MB L2; no flush"
-                         % (24 * L * points * 8 // 2 ** 20),
-                   "geometry": geom, "finite": finite},
+                   "dt_over_dr": w.dt / w.dr, "baseline_dt_over_dr": 0.5,
+                   "dt_note": "BASELINE.json says dt = 0.5 dr*; configs 2/3/5 are unstable there (DESIGN.md reading A15b, "
+                              "tests/test_oracle_stability.py) and run at inputs.stable_dt; work per update is unchanged",
+                   "precision_limbs": L, "parallelism": f"replicas x{world}", "coefficient_supply": label, "options": opts,
+                   "timing": f"median of {REPS} repetitions of {args.steps} iterations (min and all repetitions under "
+                             "ms_per_step_min / ms_per_step_all); one CUDA-graph launch per teuk_step call",
+                   "l2": f"L2 flushed (256 MiB write) between timed repetitions; inside a repetition the time loop re-reads "
+                         f"its own working set of {ws_mib} MiB (L2 is 126 MB): the HBM-bound claim is made on `large_cell`",
+                   "geometry": head["geometry"], "finite": head["finite"]},
+        "ms_per_step_min": head["ms_per_step_min"], "ms_per_step_all": head["ms_per_step_all"],
         "clocks": clocks,
         "e2e": {"value": e2e_val, "unit": "updates/s", "h2d_bytes_per_step": h2d / args.steps,
                 "d2h_bytes_per_step": d2h / args.steps,
                 "note": "teuk_set_initial(host) + teuk_step(K) + teuk_read(host) timed by wall clock; bytes are the whole "
                         "state once per K-step call divided by K"},
-        "gpu_launches": launches,
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": load_traffic(f"{w.name}"), "peak_source": peak_src, "kernel": "step_kernel_f64_rc" if recompute else ("step2_kernel_f64_tma" if "time_block=2" in opt_set and L == 1 else "step_kernel_f64_tma" if L == 1 else f"step_kernel<{L}>"),
-                     "algorithmic_bytes_per_update": bytes_per_update},
+        "gpu_launches": r["launches"],
+        "roofline": head["roofline"],
     }
-    if not args.no_extra and world == 1:
+    if extra:
+        line["cpu_baseline"] = head["cpu_baseline"]
+        k10 = max(50, args.steps // 10)
+        if L == 1 and not chose:
+            # the other coefficient supply of the primary workload (H1b): stored planes, 192 B/update
+            line["stored_planes"], _ = measure(torch, teuk, w, args.steps, args.warmup, other + ["coef_variant=0"],
+                                               peak, peak_src, pipe, with_cpu=False, with_e2e=False)
+            # above L2: sweep cell 65536 x 64 (working set 576 MiB semi-recompute / 1 GiB stored planes), both supplies
+            big = {}
+            for tag, o2 in (("semi_recompute", ["coef_variant=1"]), ("stored_planes", ["coef_variant=0"])):
+                big[tag], _ = measure(torch, teuk, "sweep:65536x64", max(20, args.steps // 4), 10, other + o2,
+                                      peak, peak_src, pipe, with_cpu=False, with_e2e=False)
+            line["large_cell"] = big
+        # dd and qd (BASELINE.json configs[2], configs[3]): rate, FP64-pipe roofline, e2e and the oracle beside each
         per = {}
-        fp = {k: teuk.bench_fp64(k) for k in ("dfma", "dadd", "dmul")}
-        for name, k_steps in (("cfg3", max(50, args.steps // 10)), ("cfg4", max(50, args.steps // 10))):
-            wx = workload(name)
-            msx, lx, gx, fx = time_device(torch, teuk, wx, k_steps, 20, args.option)
-            upsx = wx.n_r * wx.n_theta * k_steps / (msx * 1e-3)
-            per[name] = {"precision_limbs": wx.precision, "n_r": wx.n_r, "n_theta": wx.n_theta, "steps": k_steps,
-                         "updates_per_s": upsx, "ms_per_step": msx / k_steps, "geometry": gx, "finite": fx,
-                         # FP64 instructions per update from ncu (profiles/r01e_step_kernels_ncu.md) x rate / measured DADD issue peak
-                         "roofline": {"bound": "fp64 pipe", "fp64_inst_per_update": FP64_INST_PER_UPDATE[wx.precision],
-                                      "peak_inst_per_s": fp["dadd"], "frac": upsx * FP64_INST_PER_UPDATE[wx.precision] / fp["dadd"]}}
-        # NEXT-1: the same three workloads with the 10th-order theta operator (column kernel)
+        for name in ("cfg3", "cfg4"):
+            per[name], _ = measure(torch, teuk, name, k10, 20, other, peak, peak_src, pipe)
+        line["per_precision"] = per
+        # NEXT-1: the same three workloads with the 10th-order theta operator (column kernels)
         t10 = {}
-        for name, k_steps in (("cfg2", max(50, args.steps // 10)), ("cfg3", max(50, args.steps // 10)), ("cfg4", max(50, args.steps // 10))):
+        for name in ("cfg2", "cfg3", "cfg4"):
             wx = workload(name)
             wx = wx.scaled(dt_override=0.5 * wx.dt)
-            msx, lx, gx, fx = time_device(torch, teuk, wx, k_steps, 20, list(args.option) + ["theta_order=10"])
-            t10[name] = {"precision_limbs": wx.precision, "steps": k_steps, "updates_per_s": wx.n_r * wx.n_theta * k_steps / (msx * 1e-3),
-                         "ms_per_step": msx / k_steps, "geometry": gx, "finite": fx}
+            t10[name], _ = measure(torch, teuk, wx, k10, 20, other + ["theta_order=10"], peak, peak_src, pipe,
+                                   with_cpu=False, with_e2e=False)
         line["theta_order_10"] = t10
-        # H1b variant (b): semi-recompute coefficient supply for the primary workload (80 B/update)
-        if L == 1:
-            msr, lr, gr, fr = time_device(torch, teuk, w, args.steps, args.warmup, list(args.option) + ["coef_variant=1"])
-            ach = 80.0 * points / (msr / args.steps * 1e-3) / 1e9
-            line["semi_recompute"] = {"updates_per_s": points * args.steps / (msr * 1e-3), "ms_per_step": msr / args.steps,
-                                      "algorithmic_bytes_per_update": 80.0, "hbm_frac": ach / peak, "geometry": gr, "finite": fr}
-            # H1b variant (c): full recompute (1/Sigma by rsqrt per point; state-only traffic, 64 B/update)
-            msf, lf, gf, ff = time_device(torch, teuk, w, args.steps, args.warmup, list(args.option) + ["coef_variant=2"])
-            achf = 64.0 * points / (msf / args.steps * 1e-3) / 1e9
-            line["full_recompute"] = {"updates_per_s": points * args.steps / (msf * 1e-3), "ms_per_step": msf / args.steps,
-                                      "algorithmic_bytes_per_update": 64.0, "hbm_frac": achf / peak, "geometry": gf, "finite": ff}
-            # NEXT-3: two iterations per launch (u^{n+1} and the coefficient tiles stay on the SM): 96 B/update
-            mst, lt, gt, ft = time_device(torch, teuk, w, args.steps, args.warmup, list(args.option) + ["time_block=2"])
-            acht = 96.0 * points / (mst / args.steps * 1e-3) / 1e9
-            line["time_blocked_2"] = {"updates_per_s": points * args.steps / (mst * 1e-3), "ms_per_step": mst / args.steps,
-                                      "algorithmic_bytes_per_update": 96.0, "hbm_frac": acht / peak, "gpu_launches": lt,
-                                      "geometry": gt, "finite": ft}
-        line["per_precision"] = per
-        line["fp64_pipe_peak_inst_per_s"] = fp
-        line["cpu_baseline"] = cpu_baseline(w)
+        line["fp64_pipe_peak_inst_per_s"] = {k: teuk.bench_fp64(k) for k in ("dfma", "dadd", "dmul")}
     print(json.dumps(line), flush=True)
     if d is not None:
         d.destroy_process_group()

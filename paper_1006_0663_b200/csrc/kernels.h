@@ -19,7 +19,7 @@ const void* tma_step_fn(int ti, int tj);
 const void* rc_step_fn(int ti, int tj, int full);     // full = H1b variant (c)
 const void* col_tma_fn(int ti);
 // fp64 column-march kernel (step_kernel_march.cuh): semi-recompute supply, no shared-memory tiles
-const void* march_step_fn(int rt_in_registers);
+const void* march_step_fn();
 // fp64 two-iterations-per-launch kernel (step_kernel_tb2.cuh, NEXT-3)
 const void* tb2_step_fn(int ti, int tj);
 

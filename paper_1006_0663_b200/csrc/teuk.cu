@@ -89,8 +89,8 @@ struct teuk_ctx {
     ThetaWeights tw;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
     bool use_tma = false, use_rc = false, use_col_tma = false, use_march = false;
-    int opt_march = 1, march_regs = 0;     // fp64 semi-recompute supply: column-march kernel (step_kernel_march.cuh) unless march=0
-    long march_rows_per_warp = 0, march_total_rows = 0;
+    int opt_march = 1, opt_march_chunk = 0;   // fp64 semi-recompute supply: column-march kernel (step_kernel_march.cuh) unless march=0
+    int march_strips = 0, march_chunk = 0, march_units = 0;
     CUtensorMap tm_state[2], tm_ch, tm_ci, tm_ish, tm_isi, tm_rth, tm_rti;
     // temporally blocked fp64 path (two iterations per launch, step_kernel_tb2.cuh): its own boxes, grid and smem
     bool use_tb2 = false;
@@ -409,8 +409,9 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
         c->opt_tb = v;
     } else if (!strcmp(key, "march")) {
         c->opt_march = v != 0;
-    } else if (!strcmp(key, "march_regs")) {
-        c->march_regs = v != 0;
+    } else if (!strcmp(key, "march_chunk")) {        // theta rows per work unit of the march kernel (0 = chosen by the library)
+        if (v < 0 || v > c->n_theta) return TEUK_EINVAL;
+        c->opt_march_chunk = v;
     } else if (!strcmp(key, "use_tma")) {
         c->opt_tma = v != 0;
     } else {
@@ -596,25 +597,37 @@ static int choose_geometry(teuk_ctx* c) {
         return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess ? TEUK_OK : TEUK_ECUDA;
     }
     c->use_march = false;
-    if (c->L == 1 && c->coef_variant == 1 && c->opt_march) {
-        // persistent grid: every resident warp gets an equal contiguous share of the strip-rows (strip-major)
-        const void* fn = march_step_fn(c->march_regs);
-        const size_t sm = ((size_t)4 * c->n_theta + (size_t)MARCH_WARPS * 2 * MARCH_NRT * 32) * sizeof(double);
+    if (c->L == 1 && c->coef_variant == 1 && c->opt_march && 4 * c->lay.plane < (1L << 31)) {
+        // persistent grid of resident warps; work unit = (strip of 30 columns, chunk of theta rows)
+        const void* fn = march_step_fn();
+        const size_t sm = march_smem_bytes(c->n_theta);
         int dev = 0, sms = 0, per_sm = 0;
         if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess ||
             cudaGetDevice(&dev) != cudaSuccess ||
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * MARCH_WARPS, sm) != cudaSuccess || per_sm < 1)
             return TEUK_ECUDA;
+        const int nt = c->n_theta;
         const long strips = (c->n_r + MARCH_W - 1) / MARCH_W;
-        const long total = strips * c->n_theta;
         const long capacity = (long)sms * per_sm * MARCH_WARPS;
-        long share = (total + capacity - 1) / capacity;
-        const long min_share = std::min(8, c->n_theta);            // below this the two-row theta halo dominates
-        if (share < min_share) share = min_share;
-        const long warps = (total + share - 1) / share;
-        c->march_rows_per_warp = share; c->march_total_rows = total;
-        c->ti = MARCH_W; c->tj = (int)std::min<long>(share, c->n_theta); c->smem = sm; c->threads = 32 * MARCH_WARPS;
+        // chunk length: k chunks per column; a warp's time ~ rounds x (rows + 6 rows of pipeline fill and drain + 4 halo
+        // rows when the column is cut); pick the k that minimises it (k = 1: whole columns)
+        int best_k = 1;
+        long best_cost = -1;
+        for (int k = 1; k <= std::max(1, nt / 8); ++k) {
+            const long rows = (nt + k - 1) / k;
+            const long kk = (nt + rows - 1) / rows;                 // chunks per column actually produced
+            const long rounds = (strips * kk + capacity - 1) / capacity;
+            const long cost = rounds * (rows + 6 + (kk > 1 ? 4 : 0));
+            if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_k = k; }
+        }
+        int rows = c->opt_march_chunk > 0 ? c->opt_march_chunk : (nt + best_k - 1) / best_k;
+        const long chunks = (nt + rows - 1) / rows;
+        const long units = strips * chunks;
+        if (units >= (1L << 31)) return TEUK_EINVAL;
+        const long warps = std::min(units, capacity);
+        c->march_strips = (int)strips; c->march_chunk = rows; c->march_units = (int)units;
+        c->ti = MARCH_W; c->tj = rows; c->smem = sm; c->threads = 32 * MARCH_WARPS;
         c->grid = dim3((unsigned)((warps + MARCH_WARPS - 1) / MARCH_WARPS), 1);
         c->use_march = true;
         return TEUK_OK;
@@ -693,10 +706,11 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         Q.isig_h = c->dptr(c->lay.rc_isig) + c->lay.plane;
         Q.rt = c->dptr(c->lay.rc_rt);
         Q.th = c->dptr(c->lay.rc_th);
-        Q.rows_per_warp = c->march_rows_per_warp;
-        Q.total_rows = c->march_total_rows;
+        Q.n_strips = c->march_strips;
+        Q.chunk_rows = c->march_chunk;
+        Q.n_units = c->march_units;
         void* args[] = {&P, &Q};
-        if (cudaLaunchKernel(march_step_fn(c->march_regs), c->grid, dim3(c->threads), args, c->smem, c->stream) != cudaSuccess)
+        if (cudaLaunchKernel(march_step_fn(), c->grid, dim3(c->threads), args, c->smem, c->stream) != cudaSuccess)
             return TEUK_ECUDA;
     } else if (c->use_rc || c->use_tma) {
         // programmatic dependent launch: the next step's blocks may start (and prefetch their coefficient tiles) while this
