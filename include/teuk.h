@@ -24,7 +24,8 @@ extern "C" {
 typedef struct teuk_ctx teuk_ctx;
 
 enum { TEUK_FP64 = 1, TEUK_DD = 2, TEUK_QD = 4 };      /* value == limbs per real */
-enum { TEUK_OK = 0, TEUK_EINVAL = -1, TEUK_ENOMEM = -2, TEUK_ECUDA = -3, TEUK_ESTATE = -4, TEUK_ENONFINITE = -5 };
+enum { TEUK_OK = 0, TEUK_EINVAL = -1, TEUK_ENOMEM = -2, TEUK_ECUDA = -3, TEUK_ESTATE = -4, TEUK_ENONFINITE = -5,
+       TEUK_ECAPACITY = -6 /* request exceeds a fixed, documented capacity (teuk_get_folded_static) */ };
 
 /* Bytes of device workspace teuk_create needs (two state buffers, 16 L coefficient planes, 1-D
  * tables, observer buffer for obs_capacity samples).  TEUK_EINVAL on bad sizes. */
@@ -123,6 +124,20 @@ int teuk_get_tables(teuk_ctx *, int half, double *host_out);
  * coef_variant 0 = the stored planes, 1 = rebuilt from the semi-recompute tables by a kernel, 2 = rebuilt with 1/Sigma
  * recomputed as well (full recompute). */
 int teuk_get_folded(teuk_ctx *, int half, int coef_variant, double *host_out);
+/* ALLOCATION-FREE variant of teuk_get_folded for coef_variant 1 or 2 (the two variants whose planes are rebuilt by a
+ * kernel, i.e. the ones teuk_get_folded serves through a cudaMalloc'ed scratch buffer): for callers that must not
+ * allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  The kernel's scratch is a
+ * file-scope `static __device__` array of TEUK_STATIC_SCRATCH_DOUBLES doubles (4 MiB; every GPU that loads the library
+ * holds it until the process exits); its device address is looked up once per device with cudaGetSymbolAddress.  The call
+ * allocates nothing on the device or the host (no cudaMalloc / cudaFree / allocating library routine): it clears the part
+ * of the scratch it uses, runs the same kernel as teuk_get_folded, and copies the rows straight into host_out
+ * (double[8][n_theta][rows], same layout and bit-identical values), then synchronises the handle's stream.
+ * Limit: 8 * n_theta * pitch <= TEUK_STATIC_SCRATCH_DOUBLES, pitch = n_r rounded up to 16 (e.g. 1024 x 64, 4096 x 16);
+ * larger grids return TEUK_ECAPACITY and touch nothing.  TEUK_EINVAL for non-fp64 handles or coef_variant not in {1, 2}.
+ * ALL calls (all handles, all streams of a device) share the one array, which keeps the last call's contents: calls that
+ * overlap on the GPU race -- serialise them (one stream, or an event between streams). */
+#define TEUK_STATIC_SCRATCH_DOUBLES (512 * 1024)
+int teuk_get_folded_static(teuk_ctx *, int half, int coef_variant, double *host_out);
 /* r and r - r_+ at the 2 n_r - 1 integer/half points as quad-double limbs, double[2 n_r - 1][4] each. */
 int teuk_get_radial(teuk_ctx *, double *host_r, double *host_delta);
 /* One arithmetic operation of the multiprecision layer, limbs in/out (L = 2 or 4);

@@ -1085,6 +1085,7 @@ extern "C" const char* teuk_strerror(int code) {
         case TEUK_ECUDA: return "CUDA error";
         case TEUK_ESTATE: return "call not valid in this state";
         case TEUK_ENONFINITE: return "non-finite observer sample";
+        case TEUK_ECAPACITY: return "request exceeds the fixed capacity of the static scratch array";
         default: return "unknown error";
     }
 }
@@ -1268,5 +1269,49 @@ extern "C" int teuk_bench_fp64(int kind, long iters, double* inst_per_s, void* c
     cudaFree(sink);
     if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
     *inst_per_s = (double)blocks * threads * 8.0 * (double)iters / (best * 1e-3);
+    return TEUK_OK;
+}
+
+// ------------------------------------------------------------------------------------ allocation-free entry point
+// teuk_get_folded_static (include/teuk.h): rc_tables_kernel writing into a file-scope device array instead of a
+// cudaMalloc'ed buffer.  In HOST code `g_static_scratch` is only a stand-in for the symbol, not a device address: the
+// address a kernel can use comes from cudaGetSymbolAddress, looked up once per device with that device current.
+static __device__ __align__(256) double g_static_scratch[TEUK_STATIC_SCRATCH_DOUBLES];
+
+static int static_scratch_ptr(double** out) {
+    constexpr int MAX_DEV = 64;
+    static double* ptr[MAX_DEV] = {nullptr};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEV) return TEUK_ECUDA;
+    if (!ptr[dev]) {
+        double* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress((void**)&p, g_static_scratch);      // resolves for the CURRENT device
+        if (e != cudaSuccess || !p) return cuda_fail(e, "cudaGetSymbolAddress(g_static_scratch)", __LINE__);
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return TEUK_OK;
+}
+
+extern "C" int teuk_get_folded_static(teuk_ctx* c, int half, int coef_variant, double* host_out) {
+    if (!c || !host_out || c->L != 1 || coef_variant < 1 || coef_variant > 2) return TEUK_EINVAL;
+    const size_t n = (size_t)8 * c->lay.plane;                       // 8 planes of n_theta x pitch doubles
+    if (n > (size_t)TEUK_STATIC_SCRATCH_DOUBLES) return TEUK_ECAPACITY;
+    double* scratch = nullptr;
+    int rc = static_scratch_ptr(&scratch);
+    if (rc != TEUK_OK) return rc;
+    const int rows = half ? c->n_r - 1 : c->n_r;
+    // the array keeps the previous call's contents: clear what this call uses (the kernel writes columns < rows only)
+    CK(cudaMemsetAsync(scratch, 0, n * sizeof(double), c->stream));
+    rc_tables_kernel<<<dim3((rows + 127) / 128, c->n_theta), 128, 0, c->stream>>>(
+        c->dptr(c->lay.rc_isig) + (size_t)(half ? 1 : 0) * c->lay.plane,
+        c->dptr(c->lay.rc_rt) + (size_t)(half ? 1 : 0) * RC_NT * c->lay.pitch, c->dptr(c->lay.rc_th), rows, c->n_theta,
+        c->lay.pitch, c->lay.plane, scratch, coef_variant == 2);
+    c->launches++;
+    if (cudaGetLastError() != cudaSuccess) return TEUK_ECUDA;
+    // unpad on the way out: 8 * n_theta rows of `rows` doubles, source row stride = pitch (planes are contiguous: plane = n_theta * pitch)
+    CK(cudaMemcpy2DAsync(host_out, (size_t)rows * sizeof(double), scratch, (size_t)c->lay.pitch * sizeof(double),
+                         (size_t)rows * sizeof(double), (size_t)8 * c->n_theta, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
     return TEUK_OK;
 }

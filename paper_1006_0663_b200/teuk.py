@@ -18,7 +18,8 @@ if not os.path.exists(_SO):
 lib = C.CDLL(_SO)
 
 FP64, DD, QD = 1, 2, 4
-OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENONFINITE = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENONFINITE, ECAPACITY = 0, -1, -2, -3, -4, -5, -6
+STATIC_SCRATCH_DOUBLES = 512 * 1024
 
 _dp = C.POINTER(C.c_double)
 _lp = C.POINTER(C.c_long)
@@ -49,6 +50,7 @@ SIGNATURES = {
     "teuk_strerror": (C.c_char_p, [C.c_int]),
     "teuk_get_tables": (C.c_int, [_h, C.c_int, _dp]),
     "teuk_get_folded": (C.c_int, [_h, C.c_int, C.c_int, _dp]),
+    "teuk_get_folded_static": (C.c_int, [_h, C.c_int, C.c_int, _dp]),
     "teuk_get_radial": (C.c_int, [_h, _dp, _dp]),
     "teuk_test_mp_op": (C.c_int, [C.c_int, C.c_int, _dp, _dp, _dp, C.c_long, C.c_int]),
     "teuk_test_mp_fn": (C.c_int, [C.c_int, _dp, _dp]),
@@ -233,6 +235,14 @@ class Teuk:
         rows = self.n_r - 1 if half else self.n_r
         out = np.zeros((8, self.n_theta, rows))
         _chk(lib.teuk_get_folded(self.h, int(half), coef_variant, _np(out)), "teuk_get_folded")
+        return out
+
+    def folded_static(self, half: bool, coef_variant: int, out: np.ndarray | None = None) -> np.ndarray:
+        """teuk_get_folded_static: the same planes through the library's fixed device scratch (no allocation in the call)"""
+        rows = self.n_r - 1 if half else self.n_r
+        if out is None:
+            out = np.zeros((8, self.n_theta, rows))
+        _chk(lib.teuk_get_folded_static(self.h, int(half), coef_variant, _np(out)), "teuk_get_folded_static")
         return out
 
     def radial(self):
