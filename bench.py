@@ -281,8 +281,8 @@ def load_traffic(name):
 def supply_of(options, L):
     """(label, algorithmic bytes per update) of the coefficient supply the option list selects"""
     opt = {o.replace(" ", "") for o in options}
-    if L == 1 and "coef_variant=1" in opt:
-        return "semi_recompute", SEMI_RECOMPUTE_BYTES
+    if L == 1 and ("coef_variant=1" in opt or ("theta_order=10" in opt and "use_tma=0" not in opt)):
+        return "semi_recompute", SEMI_RECOMPUTE_BYTES      # the fp64 10th-order column kernel always uses this supply
     if L == 1 and "coef_variant=2" in opt:
         return "full_recompute", 64.0
     if L == 1 and "time_block=2" in opt:
@@ -445,6 +445,7 @@ def measure(torch, teuk, name, steps, warmup, options, peak, peak_src, pipe, dis
     else:
         out["roofline"] = pipe_roofline(ups, L, pipe, 10 if "theta_order=10" in options else 2)
         out["roofline"]["kernel"] = kern
+        out["roofline"]["traffic"] = load_traffic(f"{w.name}:{kern}")
         out["hbm_frac_at_this_rate"] = ups * ALG_BYTES_PER_UPDATE[L] / 1e9 / peak
     if with_e2e:
         dt, h2d, d2h = time_e2e(torch, teuk, w, steps, options)

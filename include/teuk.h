@@ -1,7 +1,10 @@
 /* teuk.h — C ABI of libteuk.so: the time step of the m-mode-reduced 2+1D Teukolsky equation as a
  * first-order complex (Phi, Pi) system on an (r*, theta) grid in Kerr background, §III.B
  * (PAPER.md:53-112), at three precisions: fp64, double-double, quad-double.
- * Every step of the path runs in CUDA kernels for sm_100a; there is no CPU fallback.
+ * The inversion r(r*), all coefficient planes and every step of the time loop (half step, full step, boundary and
+ * polar conditions, observer extraction and interpolation) run in CUDA kernels for sm_100a; there is no CPU fallback.
+ * Host arithmetic is limited to set-up scalars and 1-D tables that do not depend on r* (theta tables, stencil and
+ * quadrature weights), evaluated once per handle in quad-double.
  *
  * Conventions
  *  - All scalar parameters are fp64 and taken as exact.  Grid: r*_i = rstar_min + i dr*,
@@ -56,13 +59,16 @@ int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_the
 /* Options, only before teuk_set_initial (else TEUK_ESTATE): "graph_steps" (even, >= 2; steps per
  * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic), "use_tma" (fp64: 1 = TMA
  * kernel, default; 0 = generic kernel), "variant" (dd/qd launch shape 0..2), "coef_variant" (0 = precomputed
- * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only; 2 = full recompute:
- * 1-D tables only, 1/Sigma = rsqrt(R^2 - a^2 Delta sin^2 theta) per point, fp64 only),
+ * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only -- the fastest fp64
+ * path (column-march kernel; "march" = 0 selects the older TMA tile kernel for the same supply, "march_chunk" = theta
+ * rows per work unit, 0 = automatic); 2 = full recompute: 1-D tables only, 1/Sigma = rsqrt(R^2 - a^2 Delta sin^2 theta)
+ * per point, fp64 only),
  * "pdl" (fp64 TMA kernels: 1 = programmatic dependent launch, the next step prefetches its half-step coefficient
  * tile while the current one drains; default 0, measured neutral), "theta_order" (2 = second-order centred theta differences, default; 10 = the 10th-order
- * 11-point operator of PAPER.md:126, needs n_theta >= 5), "time_block" (1 = one iteration per launch, default; 2 = two
+ * 11-point operator of PAPER.md:126, needs n_theta >= 5), "time_block" (1 = one iteration per launch, default; 2 = EXPERIMENT, two
  * iterations per launch on a shared-memory resident tile, fp64 stored-plane TMA path only, else TEUK_EINVAL at
- * teuk_set_initial; an odd last iteration and runs with the multipole observer use the one-iteration kernel). */
+ * teuk_set_initial; an odd last iteration and runs with the multipole observer use the one-iteration kernel; parity-green
+ * but slower than coef_variant = 1, kept for the record). */
 int teuk_set_option(teuk_ctx *, const char *key, double value);
 
 /* Observer at a fixed location: bilinear interpolation in (r*, theta) from the four

@@ -1,6 +1,7 @@
 // libteuk.so — C ABI of include/teuk.h.  Host logic only marshals arguments, lays out the caller's
-// device workspace and launches kernels; every step of the path (table setup, stepping, boundary and
-// polar conditions, observer extraction and interpolation) runs in CUDA kernels for sm_100a.
+// device workspace and launches kernels; r(r*), the coefficient planes and every step of the time loop (stepping,
+// boundary and polar conditions, observer extraction and interpolation) run in CUDA kernels for sm_100a.  Host
+// arithmetic: set-up scalars and r*-independent 1-D tables in quad-double (theta tables, stencil / quadrature weights).
 #include <cuda_runtime.h>
 
 #include <cmath>

@@ -89,8 +89,10 @@ class Teuk:
     """One solver handle (teuk_ctx).  Methods are 1:1 with the C calls."""
 
     def __init__(self, M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision, obs_capacity=0,
-                 device="cuda:0", stream=None, slab=None):
-        """slab = (i_lo, n_win): teuk_create_slab, the handle holds that column range of the n_r-node grid"""
+                 device="cuda:0", stream=None, slab=None, guard_bytes=0):
+        """slab = (i_lo, n_win): teuk_create_slab, the handle holds that column range of the n_r-node grid.
+        guard_bytes > 0 (tests): the workspace is allocated with a guard band of that many bytes on each side, filled with
+        the byte 0xA5; `guards_intact()` tells whether any kernel wrote outside the workspace it was given."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1006_0663_b200.teuk needs a CUDA device; there is no CPU fallback")
@@ -102,11 +104,16 @@ class Teuk:
         nbytes = workspace_bytes(n_r, n_theta, precision, obs_capacity)
         self.device = torch.device(device)
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            guard = (int(guard_bytes) + 255) // 256 * 256
+            self.workspace = torch.full((nbytes + 256 + 2 * guard,), 0xA5, dtype=torch.uint8, device=self.device)
             # own non-default stream unless one is given (the legacy default stream cannot be graph-captured)
             self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
+            # the tensor is allocated (and filled) on the current stream but used on self.stream from here on
+            self.stream.wait_stream(torch.cuda.current_stream(self.device))
+            self.workspace.record_stream(self.stream)
             base = self.workspace.data_ptr()
-            self._ws_ptr = (base + 255) // 256 * 256
+            self._ws_ptr = (base + 255) // 256 * 256 + guard
+            self._guard = (self._ws_ptr - base - guard, guard, self._ws_ptr - base + nbytes)   # (start of band 1, length, start of band 2)
             self.h = _h()
             if slab is None:
                 _chk(lib.teuk_create(M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision,
@@ -124,8 +131,15 @@ class Teuk:
 
     def close(self):
         if getattr(self, "h", None) and lib is not None:
-            lib.teuk_destroy(self.h)
+            lib.teuk_destroy(self.h)          # synchronises the handle's stream before the workspace can be recycled
             self.h = None
+
+    def guards_intact(self) -> bool:
+        """guard_bytes > 0 only: both guard bands around the workspace still hold their fill pattern"""
+        lo, n, hi = self._guard
+        self.stream.synchronize()
+        w = self.workspace
+        return bool((w[lo:lo + n] == 0xA5).all().item() and (w[hi:hi + n] == 0xA5).all().item()) if n else True
 
     __del__ = close
 
@@ -171,7 +185,9 @@ class Teuk:
     def read_device(self, t=None):
         if t is None:
             t = self.torch.empty((4, self.L, self.n_theta, self.n_r), dtype=self.torch.float64, device=self.device)
+        self.stream.wait_stream(self.torch.cuda.current_stream(self.device))     # `t` may still be in use there
         _chk(lib.teuk_read_device(self.h, C.c_void_p(t.data_ptr())), "teuk_read_device")
+        t.record_stream(self.stream)
         self.torch.cuda.current_stream(self.device).wait_stream(self.stream)   # consumers run there
         return t
 

@@ -85,9 +85,10 @@ def test_full_length_against_cached_oracle(teuk, k):
         pytest.xfail(f"cfg{k}: parity verified on the first {done} of {full} steps only")
 
 
-@pytest.mark.parametrize("options", [{"coef_variant": 1}, {"coef_variant": 0}],
-                         ids=["semi_recompute", "stored_planes"])
-def test_config2_full_length_both_coefficient_supplies(teuk, options):
-    """H1b: the stored-plane and the semi-recompute supply both meet 1e-12 at full length"""
+@pytest.mark.parametrize("options", [{"coef_variant": 1}, {"coef_variant": 1, "march": 0}, {"coef_variant": 0},
+                                     {"coef_variant": 2}, {"time_block": 2}],
+                         ids=["semi_recompute_march", "semi_recompute_tiles", "stored_planes", "full_recompute", "time_block_2"])
+def test_config2_full_length_every_fp64_path(teuk, options):
+    """H1b / NEXT-3: every fp64 kernel family meets the SAME 1e-12 at full length (no per-variant tolerance)"""
     done, full = _run_against_golden(teuk, 2, options)
     assert done == full

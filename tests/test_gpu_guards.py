@@ -1,0 +1,79 @@
+"""Own memory-safety and race checks of every kernel family (compute-sanitizer is closed on the GPU pool this project
+is measured on, see profiles/r02_sanitizer.md): on small ragged grids, each family runs inside a workspace surrounded by
+guard bands (no kernel may write outside the memory it was given), must leave the row padding of the state planes
+untouched, must be bit-for-bit reproducible run after run and across launch decompositions (a shared-memory or
+halo race shows up as a run-to-run difference), and the fp64 families must agree with one another to rounding."""
+import numpy as np
+import pytest
+
+from paper_1006_0663_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FAMILIES = [
+    ("f64_tma", 1, {}),
+    ("f64_generic", 1, {"use_tma": 0}),
+    ("f64_march", 1, {"coef_variant": 1}),
+    ("f64_march_chunk7", 1, {"coef_variant": 1, "march_chunk": 7}),
+    ("f64_rc", 1, {"coef_variant": 1, "march": 0}),
+    ("f64_rc_full", 1, {"coef_variant": 2}),
+    ("f64_tb2", 1, {"time_block": 2}),
+    ("dd", 2, {}),
+    ("qd", 4, {}),
+    ("f64_col_tma", 1, {"theta_order": 10}),
+    ("f64_col", 1, {"theta_order": 10, "use_tma": 0}),
+    ("dd_col", 2, {"theta_order": 10}),
+    ("qd_col", 4, {"theta_order": 10}),
+]
+
+
+@pytest.fixture(scope="module")
+def teuk():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1006_0663_b200 import teuk as t
+    return t
+
+
+def _run(teuk, L, opts, n_r, n_theta, m, steps):
+    w = inputs.config(2).scaled(n_r=n_r, n_theta=n_theta, rstar_min=-30.0, rstar_max=60.0, precision=L, m=m)
+    w = w.scaled(dt_override=0.5 * inputs.stable_dt(w))
+    u0 = inputs.random_state(n_r, n_theta, L, seed=11)
+    g = teuk.Teuk.from_workload(w, obs_capacity=steps, guard_bytes=1 << 16)
+    for k, v in opts.items():
+        g.set_option(k, v)
+    g.set_observer(7.0, 1.3, steps)
+    g.set_initial(u0)
+    g.step(steps)
+    u, ser = g.read(), g.observe(steps)
+    intact = g.guards_intact()
+    g.close()
+    return u, ser, intact
+
+
+@pytest.mark.parametrize("name,L,opts", FAMILIES, ids=[f[0] for f in FAMILIES])
+@pytest.mark.parametrize("n_r,n_theta,m", [(131, 22, 2), (67, 12, 1)])
+def test_guard_bands_and_reproducibility(teuk, name, L, opts, n_r, n_theta, m):
+    steps = 9
+    u1, s1, ok1 = _run(teuk, L, opts, n_r, n_theta, m, steps)
+    u2, s2, ok2 = _run(teuk, L, opts, n_r, n_theta, m, steps)
+    assert ok1 and ok2, "a kernel wrote outside its workspace"
+    assert np.isfinite(u1).all() and np.isfinite(s1).all() and np.abs(u1[0, 0]).max() > 0
+    assert np.array_equal(u1, u2) and np.array_equal(s1, s2), "run-to-run difference"
+    assert np.all(u1[:, :, :, 0] == 0.0) and np.all(u1[:, :, :, -1] == 0.0)      # radial Dirichlet rows
+
+
+def test_march_kernel_is_independent_of_its_work_decomposition(teuk):
+    """the column-march kernel cut into work units of different lengths (and the tile kernel of the same supply) gives
+    the same bits: no dependence on which warp handled which rows, no stale ring slots between units"""
+    ref = None
+    for opts in ({"coef_variant": 1}, {"coef_variant": 1, "march_chunk": 5}, {"coef_variant": 1, "march_chunk": 8},
+                 {"coef_variant": 1, "march_chunk": 23}, {"coef_variant": 1, "march_chunk": 37}):
+        u, ser, ok = _run(teuk, 1, opts, 333, 37, 2, 33)
+        assert ok
+        if ref is None:
+            ref = (u, ser)
+        assert np.array_equal(u, ref[0]) and np.array_equal(ser, ref[1]), opts
+    tiles, _, _ = _run(teuk, 1, {"coef_variant": 1, "march": 0}, 333, 37, 2, 33)
+    assert np.abs(tiles - ref[0]).max() <= 1e-13 * np.abs(ref[0]).max()

@@ -525,37 +525,15 @@ def test_config2_prefix_full_grid_fp64(teuk):
     assert max(serr.values()) <= TOL[1] or np.abs(o.observe(steps)).max() < 1e-300
 
 
-@pytest.mark.skipif(os.environ.get("TEUK_FULL_LENGTH") != "1",
-                    reason="7 minutes of host time for the full-grid oracle; set TEUK_FULL_LENGTH=1 "
-                           "(measured on B200: Phi 2.1e-14, Pi 8.9e-13, observer 2.8e-14; DESIGN.md section 5)")
-def test_config2_full_length_fp64(teuk):
-    """BASELINE.json config 2 at full size AND full length (20000 steps) against the full-grid oracle,
-    for both coefficient supplies (stored planes; semi-recompute) and the two-iterations-per-launch kernel."""
-    w = inputs.config(2)
-    u0 = inputs.initial_state(w)
-    o = run_oracle(w, u0, w.steps, observer=w.observer)
-    ref, sref = o.read(), o.observe(w.steps)
-    res = {}
-    variants = {"stored planes": {"coef_variant": 0}, "semi-recompute": {"coef_variant": 1}, "full recompute": {"coef_variant": 2},
-                "time_block=2": {"time_block": 2}}
-    for name, opts in variants.items():
-        g = run_gpu(teuk, w, u0, w.steps, observer=w.observer, options=opts)
-        res[name] = (oracle.rel_linf(g.read(), ref), series_err(g.observe(w.steps), sref))
-        print("cfg2 full length,", name, ": state", res[name][0], "observer", res[name][1])
-    for name in variants:
-        # the full-recompute supply (H1b variant (c)) does NOT meet the 1e-12 bar at full length (measured Pi 1.3e-12: its
-        # fp64-evaluated 1/Sigma carries ~1 ulp of time-independent error instead of 0.5): recorded as such in DESIGN.md,
-        # checked here only against a looser bound so that a regression still shows
-        bound = 2e-12 if name == "full recompute" else TOL[1]
-        assert max(res[name][0].values()) <= bound, name
-        assert max(res[name][1].values()) <= bound, name
+# Config 2 at full size and FULL length against the oracle, for every fp64 kernel family at the same 1e-12: see
+# tests/test_gpu_golden.py (un-gated; the oracle side is cached in tests/golden/cfg2_full.npz).
 
 
 @pytest.mark.parametrize("cfg", [3, 4])
 def test_full_length_precision_ladder_on_gpu(teuk, cfg):
-    """BASELINE.json configs 3 and 4 at FULL size and FULL length (20000 / 50000 steps), which the oracle cannot reach
-    in test time: the same run at the three precisions must form a ladder (a property that holds at any size) —
-    fp64 agrees with dd to fp64 accuracy, dd with qd to dd accuracy — and stay finite.  Observer series included."""
+    """SMOKE, NOT PARITY (it compares the CUDA path with itself; parity at full length is tests/test_gpu_golden.py):
+    configs 3 and 4 at full size and full length at the three precisions must form a ladder -- fp64 agrees with dd to
+    fp64 accuracy, dd with qd to dd accuracy -- and stay finite.  Observer series included."""
     w = inputs.config(cfg)
     u0 = inputs.initial_state(w)
     out = {}
@@ -584,10 +562,9 @@ def test_full_length_precision_ladder_on_gpu(teuk, cfg):
                            "(TEUK_FULL_STEPS_CFG3 / TEUK_FULL_STEPS_CFG4 change the prefix; results: DESIGN.md section 5)")
 @pytest.mark.parametrize("cfg", [3, 4])
 def test_config3_config4_full_grid_long_runs(teuk, cfg):
-    """BASELINE.json configs 3 (dd) and 4 (qd) at FULL size against the FULL-GRID oracle (no windows), observer series
-    included, over a prefix: the exact-then-round oracle advances about 3.5e5 dd or qd updates/s on 16 cores (3 s per
-    iteration of config 3), so the full 20000 / 50000 steps would take 17 / 11 hours; the rest of the run stays covered
-    by the full-size windowed tests and the full-length precision ladder."""
+    """BASELINE.json configs 3 (dd) and 4 (qd) at FULL size against the FULL-GRID oracle (no windows) in its ARBITRATION
+    tier (exact-then-round arithmetic, about 3.5e5 updates/s on 16 cores), observer series included, over a prefix.
+    The full-length comparison (fast oracle tier, cached) is tests/test_gpu_golden.py."""
     w = inputs.config(cfg)
     steps = int(os.environ.get(f"TEUK_FULL_STEPS_CFG{cfg}", {3: 200, 4: 400}[cfg]))
     u0 = inputs.initial_state(w)
