@@ -109,7 +109,8 @@ int teuk_observe(teuk_ctx *, double *host_out, long max_samples, long *count);
  * l_min = max(|s|, |m|), 1 <= n_ell <= 9, Fejer's first quadrature rule on the cell-centred theta grid (exact for
  * polynomials of degree < n_theta in cos(theta)), linear interpolation in r*.
  * capacity <= obs_capacity of teuk_create.  Call before teuk_set_initial or between teuk_step calls; the sample index is
- * shared with the point observer (both series restart at teuk_set_observer / teuk_set_initial). */
+ * shared with the point observer: BOTH series restart (count 0, sample 0 = the next completed iteration) at
+ * teuk_set_observer, at teuk_set_multipole_observer and at teuk_set_initial. */
 int teuk_set_multipole_observer(teuk_ctx *, double rstar_obs, int n_ell, long capacity);
 /* host_out[count][n_ell][2][L]: real and imaginary part of a_l' per completed iteration; synchronises. */
 int teuk_observe_multipoles(teuk_ctx *, double *host_out, long max_samples, long *count);

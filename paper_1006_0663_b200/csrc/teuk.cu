@@ -1038,6 +1038,10 @@ extern "C" int teuk_set_multipole_observer(teuk_ctx* c, double rstar_obs, int n_
     }
     c->drop_graphs();
     CK(cudaMemcpyAsync(c->dptr(c->lay.mp_q), q.data(), q.size() * 8, cudaMemcpyHostToDevice, c->stream));
+    // the sample counter is shared with the point observer: BOTH series restart here, as at teuk_set_observer
+    CK(cudaMemsetAsync(c->step_base(), 0, 32, c->stream));
+    c->series_origin = c->steps_done;
+    c->nonfinite = false;
     CK(cudaStreamSynchronize(c->stream));
     return TEUK_OK;
 }

@@ -640,6 +640,30 @@ def test_observer_reset_mid_run(teuk):
     assert max(series_err(got, o.observe(50)).values()) <= TOL[1]
 
 
+def test_multipole_observer_enabled_mid_run(teuk):
+    """teuk_set_multipole_observer between teuk_step calls restarts BOTH series at the current step: no stale or zero
+    leading samples, and the multipole samples are those of the oracle run from the same state"""
+    w = inputs.config(4).scaled(n_r=96, n_theta=12, rstar_min=-20.0, rstar_max=75.0, precision=1)
+    u0 = inputs.initial_state(w)
+    g = teuk.Teuk.from_workload(w, obs_capacity=40)
+    g.set_observer(40.0, 1.2, 40)
+    g.set_initial(u0)
+    g.step(13)
+    assert g.observe(40).shape[0] == 13
+    g.set_multipole_observer(30.0, 3, 40)
+    assert g.observe_multipoles(40).shape[0] == 0 and g.observe(40).shape[0] == 0
+    g.step(9)
+    got = g.observe_multipoles(40)
+    assert got.shape[0] == 9 and g.observe(40).shape[0] == 9
+    o = run_oracle(w, u0, 13)
+    o.set_multipole_observer(30.0, 3, 40)
+    o.step(9)
+    ref = o.observe_multipoles(40)
+    assert ref.shape == got.shape
+    scale = np.abs(ref).max()
+    assert scale > 0 and np.abs(got - ref).max() <= TOL[1] * scale
+
+
 def test_edge_cases_and_errors(teuk):
     import ctypes
     # smallest legal grid, odd m, zero steps
