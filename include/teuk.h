@@ -30,17 +30,25 @@ enum { TEUK_FP64 = 1, TEUK_DD = 2, TEUK_QD = 4 };      /* value == limbs per rea
 enum { TEUK_OK = 0, TEUK_EINVAL = -1, TEUK_ENOMEM = -2, TEUK_ECUDA = -3, TEUK_ESTATE = -4, TEUK_ENONFINITE = -5,
        TEUK_ECAPACITY = -6 /* request exceeds a fixed, documented capacity (teuk_get_folded_static) */ };
 
-/* Bytes of device workspace teuk_create needs (two state buffers, 16 L coefficient planes, 1-D
- * tables, observer buffer for obs_capacity samples).  TEUK_EINVAL on bad sizes. */
-int teuk_workspace_bytes(int n_r, int n_theta, int precision, long obs_capacity, size_t *bytes);
+/* Bytes of device workspace teuk_create needs for the same (n_r, n_theta, precision, coef_variant, obs_capacity): two
+ * state buffers, the coefficient supplies selected by coef_variant, 1-D tables, observer buffers for obs_capacity samples.
+ * coef_variant = which coefficient supplies are RESIDENT in the workspace (H1b):
+ *   -1  all of them (fp64: 16 stored planes + the two 1/Sigma planes + r-tables), the supply is then chosen per run with
+ *       teuk_set_option("coef_variant", ...) and the test hooks can compare them on one handle;
+ *    0  the 16 L precomputed folded planes only (the only supply of dd / qd handles);
+ *    1, 2  fp64 only: the recompute tables only (two 1/Sigma planes + 1-D tables) -- no stored planes, 128 MiB less on
+ *       config 2, 2 GiB less on the 65536 x 256 sweep cell; the handle then steps with that variant and rejects the others.
+ * TEUK_EINVAL on bad sizes or variant. */
+int teuk_workspace_bytes(int n_r, int n_theta, int precision, int coef_variant, long obs_capacity, size_t *bytes);
 
 /* Build the time-independent tables on the device (r(r*) from Eq. (2); b from Eqs. (6)-(7)
  * PAPER.md:76-80; alpha, gamma, W, kappa of S in Eq. (12) PAPER.md:98 derived from Eq. (1), see
  * DESIGN.md §3), evaluated in quad-double and rounded to L limbs.  M > 0, |a| < M, n_r >= 3,
- * n_theta >= 2, dt > 0, rstar_min < rstar_max, precision in {1, 2, 4}; else TEUK_EINVAL.
+ * n_theta >= 2, dt > 0, rstar_min < rstar_max, precision in {1, 2, 4}, coef_variant as for teuk_workspace_bytes
+ * (only the resident supplies are built); else TEUK_EINVAL.
  * obs_capacity = number of observer samples the workspace was sized for. */
 int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double rstar_min, double rstar_max,
-                double dt, int precision, void *d_workspace, size_t workspace_bytes, long obs_capacity,
+                double dt, int precision, int coef_variant, void *d_workspace, size_t workspace_bytes, long obs_capacity,
                 void *cuda_stream, teuk_ctx **out);
 
 /* Radial slab of the same problem (the paper's own domain decomposition):
@@ -53,8 +61,8 @@ int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double r
  * column per iteration) - the caller keeps a halo and refreshes it with teuk_write_columns_device (see
  * paper_1006_0663_b200/slabs.py).  0 <= i_lo, i_lo + n_win <= n_r_global, n_win >= 3; workspace sized for n_win. */
 int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_theta, double rstar_min, double rstar_max,
-                     double dt, int precision, int i_lo, int n_win, void *d_workspace, size_t workspace_bytes,
-                     long obs_capacity, void *cuda_stream, teuk_ctx **out);
+                     double dt, int precision, int coef_variant, int i_lo, int n_win, void *d_workspace,
+                     size_t workspace_bytes, long obs_capacity, void *cuda_stream, teuk_ctx **out);
 
 /* Options, only before teuk_set_initial (else TEUK_ESTATE): "graph_steps" (even, >= 2; steps per
  * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic), "use_tma" (fp64: 1 = TMA

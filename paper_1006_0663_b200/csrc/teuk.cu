@@ -43,7 +43,11 @@ struct Layout {
     size_t state_a, state_b, coef_i, coef_h, cj, r_tab, d_tab, sin_tab, cos_tab, obs_raw, obs_out, scalars, rc_rt, rc_isig, rc_th, mp_q, mp_series, total;
 };
 
-static Layout make_layout(int n_r, int n_theta, int L, long cap) {
+// cv = coefficient supplies resident in the workspace: -1 all (switchable with teuk_set_option), 0 stored planes only,
+// 1 / 2 recompute tables only (fp64)
+static inline bool cv_has_planes(int L, int cv) { return L > 1 || cv <= 0; }
+static inline bool cv_has_rc(int L, int cv) { return L == 1 && cv != 0; }
+static Layout make_layout(int n_r, int n_theta, int L, long cap, int cv) {
     Layout y;
     y.pitch = (int)align_up((size_t)n_r, 16);
     y.plane = (long)y.pitch * n_theta;
@@ -55,8 +59,8 @@ static Layout make_layout(int n_r, int n_theta, int L, long cap) {
     };
     y.state_a = take((size_t)4 * L * y.plane);
     y.state_b = take((size_t)4 * L * y.plane);
-    y.coef_i = take((size_t)8 * L * y.plane);
-    y.coef_h = take((size_t)8 * L * y.plane);
+    y.coef_i = take(cv_has_planes(L, cv) ? (size_t)8 * L * y.plane : 1);
+    y.coef_h = take(cv_has_planes(L, cv) ? (size_t)8 * L * y.plane : 1);
     y.cj = take((size_t)L * n_theta);
     y.r_tab = take((size_t)4 * (2 * n_r - 1));
     y.d_tab = take((size_t)4 * (2 * n_r - 1));
@@ -66,9 +70,9 @@ static Layout make_layout(int n_r, int n_theta, int L, long cap) {
     y.obs_out = take((size_t)(cap > 0 ? cap : 1) * 4 * L);
     y.scalars = take(8);
     // semi-recompute supply (fp64 only): r-tables [2][16][pitch], isig planes [2][n_theta][pitch], theta tables [3][n_theta]
-    y.rc_rt = take(L == 1 ? (size_t)2 * RC_NT * y.pitch : 1);
-    y.rc_isig = take(L == 1 ? (size_t)2 * y.plane : 1);
-    y.rc_th = take(L == 1 ? (size_t)3 * n_theta : 1);
+    y.rc_rt = take(cv_has_rc(L, cv) ? (size_t)2 * RC_NT * y.pitch : 1);
+    y.rc_isig = take(cv_has_rc(L, cv) ? (size_t)2 * y.plane : 1);
+    y.rc_th = take(cv_has_rc(L, cv) ? (size_t)3 * n_theta : 1);
     // multipole-projection observer (NEXT-2): weights [9][L][n_theta], series [cap][9][2][L]
     y.mp_q = take((size_t)MP_MAX_ELL * L * n_theta);
     y.mp_series = take((size_t)(cap > 0 ? cap : 1) * MP_MAX_ELL * 2 * L);
@@ -80,6 +84,8 @@ struct teuk_ctx {
     double M, a, rmin, rmax, dt;
     int s, m, n_r, n_theta, L;
     int i_lo = 0, n_r_global = 0;      // radial slab: local column i <-> global column i_lo + i
+    int create_variant = -1;           // supplies resident in the workspace (see make_layout)
+    bool has_planes = true, has_rc = false;
     long cap_alloc;
     char* ws;
     Layout lay;
@@ -244,9 +250,11 @@ static bool valid_sizes(int n_r, int n_theta, int precision, long cap) {
            (long)n_r * n_theta < (1L << 31);
 }
 
-extern "C" int teuk_workspace_bytes(int n_r, int n_theta, int precision, long obs_capacity, size_t* bytes) {
-    if (!bytes || !valid_sizes(n_r, n_theta, precision, obs_capacity)) return TEUK_EINVAL;
-    *bytes = make_layout(n_r, n_theta, precision, obs_capacity).total;
+static bool valid_variant(int precision, int cv) { return cv >= -1 && cv <= 2 && (cv < 1 || precision == 1); }
+
+extern "C" int teuk_workspace_bytes(int n_r, int n_theta, int precision, int coef_variant, long obs_capacity, size_t* bytes) {
+    if (!bytes || !valid_sizes(n_r, n_theta, precision, obs_capacity) || !valid_variant(precision, coef_variant)) return TEUK_EINVAL;
+    *bytes = make_layout(n_r, n_theta, precision, obs_capacity, coef_variant).total;
     return TEUK_OK;
 }
 
@@ -267,21 +275,23 @@ static int launch_coef_any(teuk_ctx* c, int half, int fold, double* out) {
 
 // one handle = columns [i_lo, i_lo + n_r) of the uniform grid of n_r_global nodes on [rstar_min, rstar_max]
 static int create_impl(double M, double a, int s, int m, int n_r_global, int i_lo, int n_r, int n_theta, double rstar_min,
-                       double rstar_max, double dt, int precision, void* d_workspace, size_t workspace_bytes,
+                       double rstar_max, double dt, int precision, int cv, void* d_workspace, size_t workspace_bytes,
                        long obs_capacity, void* cuda_stream, teuk_ctx** out) {
-    if (!out || !d_workspace || !valid_sizes(n_r, n_theta, precision, obs_capacity)) return TEUK_EINVAL;
+    if (!out || !d_workspace || !valid_sizes(n_r, n_theta, precision, obs_capacity) || !valid_variant(precision, cv)) return TEUK_EINVAL;
     if (i_lo < 0 || (long)i_lo + n_r > n_r_global || n_r_global >= (1 << 29)) return TEUK_EINVAL;
     if (!(M > 0) || !(std::fabs(a) < M) || !(dt > 0) || !(rstar_min < rstar_max)) return TEUK_EINVAL;
     if (!std::isfinite(M) || !std::isfinite(a) || !std::isfinite(dt) || !std::isfinite(rstar_min) ||
         !std::isfinite(rstar_max))
         return TEUK_EINVAL;
-    Layout lay = make_layout(n_r, n_theta, precision, obs_capacity);
+    Layout lay = make_layout(n_r, n_theta, precision, obs_capacity, cv);
     if (workspace_bytes < lay.total || ((size_t)d_workspace % 256) != 0) return TEUK_EINVAL;
     teuk_ctx* c = new (std::nothrow) teuk_ctx();
     if (!c) return TEUK_ENOMEM;
     c->M = M; c->a = a; c->s = s; c->m = m; c->n_r = n_r; c->n_theta = n_theta; c->L = precision;
     c->rmin = rstar_min; c->rmax = rstar_max; c->dt = dt; c->cap_alloc = obs_capacity;
     c->i_lo = i_lo; c->n_r_global = n_r_global;
+    c->create_variant = cv; c->has_planes = cv_has_planes(precision, cv); c->has_rc = cv_has_rc(precision, cv);
+    c->coef_variant = cv < 0 ? 0 : cv;
     c->ws = (char*)d_workspace; c->lay = lay; c->stream = (cudaStream_t)cuda_stream;
 
     // ---- host scalars in quad-double
@@ -337,7 +347,7 @@ static int create_impl(double M, double a, int s, int m, int n_r_global, int i_l
     radial_kernel<<<(npts + 63) / 64, 64, 0, c->stream>>>(C, c->dptr(lay.r_tab), c->dptr(lay.d_tab));
     c->launches++;
     if (cudaGetLastError() != cudaSuccess) return fail(TEUK_ECUDA);
-    if (precision == 1) {
+    if (c->has_rc) {
         // semi-recompute supply: theta tables on the host in quad-double, r-tables and isig planes on the device
         std::vector<double> th((size_t)3 * n_theta);
         for (int j = 0; j < n_theta; ++j) {
@@ -360,25 +370,28 @@ static int create_impl(double M, double a, int s, int m, int n_r_global, int i_l
         c->launches += 3;
         if (cudaGetLastError() != cudaSuccess) return fail(TEUK_ECUDA);
     }
-    if ((rc = launch_coef_any(c, 0, 1, c->dptr(lay.coef_i))) != TEUK_OK) return fail(rc);
-    if ((rc = launch_coef_any(c, 1, 1, c->dptr(lay.coef_h))) != TEUK_OK) return fail(rc);
+    if (c->has_planes) {
+        if ((rc = launch_coef_any(c, 0, 1, c->dptr(lay.coef_i))) != TEUK_OK) return fail(rc);
+        if ((rc = launch_coef_any(c, 1, 1, c->dptr(lay.coef_h))) != TEUK_OK) return fail(rc);
+    }
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) return fail(TEUK_ECUDA);
     *out = c;
     return TEUK_OK;
 }
 
 extern "C" int teuk_create(double M, double a, int s, int m, int n_r, int n_theta, double rstar_min, double rstar_max,
-                           double dt, int precision, void* d_workspace, size_t workspace_bytes, long obs_capacity,
-                           void* cuda_stream, teuk_ctx** out) {
-    return create_impl(M, a, s, m, n_r, 0, n_r, n_theta, rstar_min, rstar_max, dt, precision, d_workspace, workspace_bytes,
-                       obs_capacity, cuda_stream, out);
+                           double dt, int precision, int coef_variant, void* d_workspace, size_t workspace_bytes,
+                           long obs_capacity, void* cuda_stream, teuk_ctx** out) {
+    return create_impl(M, a, s, m, n_r, 0, n_r, n_theta, rstar_min, rstar_max, dt, precision, coef_variant, d_workspace,
+                       workspace_bytes, obs_capacity, cuda_stream, out);
 }
 
 extern "C" int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_theta, double rstar_min,
-                                double rstar_max, double dt, int precision, int i_lo, int n_win, void* d_workspace,
-                                size_t workspace_bytes, long obs_capacity, void* cuda_stream, teuk_ctx** out) {
-    return create_impl(M, a, s, m, n_r_global, i_lo, n_win, n_theta, rstar_min, rstar_max, dt, precision, d_workspace,
-                       workspace_bytes, obs_capacity, cuda_stream, out);
+                                double rstar_max, double dt, int precision, int coef_variant, int i_lo, int n_win,
+                                void* d_workspace, size_t workspace_bytes, long obs_capacity, void* cuda_stream,
+                                teuk_ctx** out) {
+    return create_impl(M, a, s, m, n_r_global, i_lo, n_win, n_theta, rstar_min, rstar_max, dt, precision, coef_variant,
+                       d_workspace, workspace_bytes, obs_capacity, cuda_stream, out);
 }
 
 extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
@@ -401,6 +414,7 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
         c->theta_order = v;
     } else if (!strcmp(key, "coef_variant")) {
         if (v < 0 || v > 2 || (v >= 1 && c->L != 1)) return TEUK_EINVAL;
+        if (v == 0 ? !c->has_planes : !c->has_rc) return TEUK_EINVAL;      // that supply is not resident in this handle's workspace
         c->coef_variant = v;
     } else if (!strcmp(key, "variant")) {
         if (v < 0 || v > 2) return TEUK_EINVAL;
@@ -573,13 +587,13 @@ static int choose_geometry(teuk_ctx* c) {
     if (c->theta_order == 10) {
         fill_theta_weights(c->tw);
         c->use_col_tma = false;
-        if (c->L == 1 && c->opt_tma && c->n_theta <= 256 && (c->opt_ti == 0 || c->opt_ti == 8 || c->opt_ti == 12 || c->opt_ti == 16)) {
+        if (c->L == 1 && c->has_rc && c->opt_tma && c->n_theta <= 256 && (c->opt_ti == 0 || c->opt_ti == 8 || c->opt_ti == 12 || c->opt_ti == 16)) {
             // fp64: TMA column kernel with the semi-recompute coefficient supply (always, whatever coef_variant says)
             bool ok = c->opt_ti == 16 ? setup_col_tma<16>(c) : c->opt_ti == 12 ? setup_col_tma<12>(c) : setup_col_tma<8>(c);
             cudaGetLastError();
             if (ok) { c->use_col_tma = true; return TEUK_OK; }
         }
-        if (c->coef_variant != 0) return TEUK_EINVAL;
+        if (c->coef_variant != 0 || !c->has_planes) return TEUK_EINVAL;
         int ti = c->opt_ti;
         if (ti == 0) {
             // largest tile within the shared-memory budget: 3 blocks/SM for qd (72 KB each), 2 blocks/SM otherwise (100 KB)
@@ -640,6 +654,7 @@ static int choose_geometry(teuk_ctx* c) {
         c->use_rc = true;
         return TEUK_OK;
     }
+    if (!c->has_planes) return TEUK_EINVAL;      // every path below reads the stored coefficient planes
     if (c->L == 1 && c->opt_tma && (c->opt_ti == 0 || c->opt_ti == 32) && (c->opt_tj == 0 || c->opt_tj == 8 || c->opt_tj == 16)) {
         bool ok = (c->opt_tj == 8) ? setup_tma<32, 8>(c) : setup_tma<32, 16>(c);
         cudaGetLastError();
@@ -1130,6 +1145,7 @@ __global__ void rc_tables_kernel(const double* __restrict__ isig, const double* 
 
 extern "C" int teuk_get_folded(teuk_ctx* c, int half, int coef_variant, double* host_out) {
     if (!c || !host_out || c->L != 1 || coef_variant < 0 || coef_variant > 2) return TEUK_EINVAL;
+    if (coef_variant == 0 ? !c->has_planes : !c->has_rc) return TEUK_EINVAL;      // supply not resident in this handle
     int rows = half ? c->n_r - 1 : c->n_r;
     size_t n = (size_t)8 * c->lay.plane;
     std::vector<double> h(n);
@@ -1299,7 +1315,7 @@ static int static_scratch_ptr(double** out) {
 }
 
 extern "C" int teuk_get_folded_static(teuk_ctx* c, int half, int coef_variant, double* host_out) {
-    if (!c || !host_out || c->L != 1 || coef_variant < 1 || coef_variant > 2) return TEUK_EINVAL;
+    if (!c || !host_out || c->L != 1 || coef_variant < 1 || coef_variant > 2 || !c->has_rc) return TEUK_EINVAL;
     const size_t n = (size_t)8 * c->lay.plane;                       // 8 planes of n_theta x pitch doubles
     if (n > (size_t)TEUK_STATIC_SCRATCH_DOUBLES) return TEUK_ECAPACITY;
     double* scratch = nullptr;

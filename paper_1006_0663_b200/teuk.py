@@ -25,12 +25,12 @@ _dp = C.POINTER(C.c_double)
 _lp = C.POINTER(C.c_long)
 _h = C.c_void_p
 SIGNATURES = {
-    "teuk_workspace_bytes": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_long, C.POINTER(C.c_size_t)]),
+    "teuk_workspace_bytes": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_long, C.POINTER(C.c_size_t)]),
     "teuk_create": (C.c_int, [C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
-                              C.c_double, C.c_int, C.c_void_p, C.c_size_t, C.c_long, C.c_void_p, C.POINTER(_h)]),
+                              C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_long, C.c_void_p, C.POINTER(_h)]),
     "teuk_create_slab": (C.c_int, [C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
-                                   C.c_double, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_long, C.c_void_p,
-                                   C.POINTER(_h)]),
+                                   C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_long,
+                                   C.c_void_p, C.POINTER(_h)]),
     "teuk_set_option": (C.c_int, [_h, C.c_char_p, C.c_double]),
     "teuk_set_observer": (C.c_int, [_h, C.c_double, C.c_double, C.c_long]),
     "teuk_set_initial": (C.c_int, [_h, _dp, C.c_int]),
@@ -79,9 +79,10 @@ def _np(a: np.ndarray):
     return a.ctypes.data_as(_dp)
 
 
-def workspace_bytes(n_r: int, n_theta: int, precision: int, obs_capacity: int) -> int:
+def workspace_bytes(n_r: int, n_theta: int, precision: int, obs_capacity: int, coef_variant: int = -1) -> int:
+    """coef_variant: -1 = all coefficient supplies resident (default), 0 = stored planes only, 1 / 2 = recompute tables only"""
     out = C.c_size_t(0)
-    _chk(lib.teuk_workspace_bytes(n_r, n_theta, precision, obs_capacity, C.byref(out)), "teuk_workspace_bytes")
+    _chk(lib.teuk_workspace_bytes(n_r, n_theta, precision, coef_variant, obs_capacity, C.byref(out)), "teuk_workspace_bytes")
     return out.value
 
 
@@ -89,7 +90,7 @@ class Teuk:
     """One solver handle (teuk_ctx).  Methods are 1:1 with the C calls."""
 
     def __init__(self, M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision, obs_capacity=0,
-                 device="cuda:0", stream=None, slab=None, guard_bytes=0):
+                 device="cuda:0", stream=None, slab=None, guard_bytes=0, coef_variant=-1):
         """slab = (i_lo, n_win): teuk_create_slab, the handle holds that column range of the n_r-node grid.
         guard_bytes > 0 (tests): the workspace is allocated with a guard band of that many bytes on each side, filled with
         the byte 0xA5; `guards_intact()` tells whether any kernel wrote outside the workspace it was given."""
@@ -101,7 +102,8 @@ class Teuk:
         if slab is not None:
             i_lo, n_r = int(slab[0]), int(slab[1])
         self.n_r, self.n_theta, self.L, self.i_lo, self.n_r_global = n_r, n_theta, precision, i_lo, n_r_global
-        nbytes = workspace_bytes(n_r, n_theta, precision, obs_capacity)
+        nbytes = workspace_bytes(n_r, n_theta, precision, obs_capacity, coef_variant)
+        self.workspace_nbytes = nbytes
         self.device = torch.device(device)
         with torch.cuda.device(self.device):
             guard = (int(guard_bytes) + 255) // 256 * 256
@@ -116,11 +118,12 @@ class Teuk:
             self._guard = (self._ws_ptr - base - guard, guard, self._ws_ptr - base + nbytes)   # (start of band 1, length, start of band 2)
             self.h = _h()
             if slab is None:
-                _chk(lib.teuk_create(M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision,
+                _chk(lib.teuk_create(M, a, s, m, n_r, n_theta, rstar_min, rstar_max, dt, precision, coef_variant,
                                      C.c_void_p(self._ws_ptr), nbytes, obs_capacity,
                                      C.c_void_p(self.stream.cuda_stream), C.byref(self.h)), "teuk_create")
             else:
-                _chk(lib.teuk_create_slab(M, a, s, m, n_r_global, n_theta, rstar_min, rstar_max, dt, precision, i_lo, n_r,
+                _chk(lib.teuk_create_slab(M, a, s, m, n_r_global, n_theta, rstar_min, rstar_max, dt, precision, coef_variant,
+                                          i_lo, n_r,
                                           C.c_void_p(self._ws_ptr), nbytes, obs_capacity,
                                           C.c_void_p(self.stream.cuda_stream), C.byref(self.h)), "teuk_create_slab")
 

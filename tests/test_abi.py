@@ -34,12 +34,20 @@ def test_library_exports_every_declared_symbol():
 def test_argument_validation_without_gpu():
     teuk = pytest.importorskip("paper_1006_0663_b200.teuk")
     out = ctypes.c_size_t(0)
-    assert teuk.lib.teuk_workspace_bytes(2, 16, 1, 0, ctypes.byref(out)) == teuk.EINVAL
-    assert teuk.lib.teuk_workspace_bytes(512, 16, 3, 0, ctypes.byref(out)) == teuk.EINVAL
-    assert teuk.lib.teuk_workspace_bytes(512, 16, 1, 2000, ctypes.byref(out)) == teuk.OK
+    assert teuk.lib.teuk_workspace_bytes(2, 16, 1, -1, 0, ctypes.byref(out)) == teuk.EINVAL
+    assert teuk.lib.teuk_workspace_bytes(512, 16, 3, -1, 0, ctypes.byref(out)) == teuk.EINVAL
+    assert teuk.lib.teuk_workspace_bytes(512, 16, 1, 3, 0, ctypes.byref(out)) == teuk.EINVAL      # no such supply
+    assert teuk.lib.teuk_workspace_bytes(512, 16, 2, 1, 0, ctypes.byref(out)) == teuk.EINVAL      # recompute supplies are fp64 only
+    assert teuk.lib.teuk_workspace_bytes(512, 16, 1, -1, 2000, ctypes.byref(out)) == teuk.OK
     # two state buffers + 16 coefficient planes of 16 x 512 doubles at least
     assert out.value >= (8 + 16) * 512 * 16 * 8
     assert teuk.workspace_bytes(16384, 64, 2, 0) >= 2 * (8 + 16) * 16384 * 64 * 8
+    # H1b: a handle created for the semi-recompute supply carries no stored planes: state (2 x 32 MiB) + two 1/Sigma planes
+    # (16 MiB) + small tables on config 2, instead of those + 128 MiB
+    plane = 16384 * 64 * 8
+    both, planes_only, rc_only = (teuk.workspace_bytes(16384, 64, 1, 0, cv) for cv in (-1, 0, 1))
+    assert both - rc_only >= 16 * plane - 4096 and both - planes_only >= 2 * plane      # (256-byte placeholders remain)
+    assert 10 * plane <= rc_only < 11 * plane and teuk.workspace_bytes(16384, 64, 1, 0, 2) == rc_only
     h = ctypes.c_void_p()
-    assert teuk.lib.teuk_create(1.0, 1.0, 0, 0, 64, 8, -10.0, 10.0, 0.1, 1, None, 0, 0, None, ctypes.byref(h)) == teuk.EINVAL
+    assert teuk.lib.teuk_create(1.0, 1.0, 0, 0, 64, 8, -10.0, 10.0, 0.1, 1, -1, None, 0, 0, None, ctypes.byref(h)) == teuk.EINVAL
     assert teuk.lib.teuk_strerror(teuk.ESTATE).decode().startswith("call not valid")

@@ -77,3 +77,47 @@ def test_march_kernel_is_independent_of_its_work_decomposition(teuk):
         assert np.array_equal(u, ref[0]) and np.array_equal(ser, ref[1]), opts
     tiles, _, _ = _run(teuk, 1, {"coef_variant": 1, "march": 0}, 333, 37, 2, 33)
     assert np.abs(tiles - ref[0]).max() <= 1e-13 * np.abs(ref[0]).max()
+
+
+def test_handle_created_for_one_supply_only(teuk):
+    """teuk_create(coef_variant = 1): no stored planes in the workspace (H1b); same bits as the all-supplies
+    handle stepping with that variant; the supplies that are not resident are refused"""
+    n_r, n_theta, steps = 300, 24, 21
+    w = inputs.config(2).scaled(n_r=n_r, n_theta=n_theta, rstar_min=-30.0, rstar_max=60.0, precision=1)
+    w = w.scaled(dt_override=inputs.stable_dt(w))
+    u0 = inputs.random_state(n_r, n_theta, 1, seed=3)
+    out = {}
+    for cv in (-1, 1, 2, 0):
+        g = teuk.Teuk.from_workload(w, obs_capacity=steps, guard_bytes=1 << 16, coef_variant=cv)
+        if cv == -1:
+            g.set_option("coef_variant", 1)
+            full_bytes = g.workspace_nbytes
+        else:
+            plane = n_theta * ((n_r + 15) // 16 * 16) * 8
+            assert full_bytes - g.workspace_nbytes >= (16 if cv else 2) * plane - 4096
+            for other in ({0, 1, 2} - {cv} if cv == 0 else {0}):
+                with pytest.raises(teuk.TeukError) as e:
+                    g.set_option("coef_variant", other)
+                assert e.value.code == teuk.EINVAL
+            with pytest.raises(teuk.TeukError):
+                g.folded(False, 0 if cv else 1)
+        g.set_observer(7.0, 1.3, steps)
+        g.set_initial(u0)
+        g.step(steps)
+        out[cv] = (g.read(), g.observe(steps))
+        assert g.guards_intact()
+        g.close()
+    assert np.array_equal(out[1][0], out[-1][0]) and np.array_equal(out[1][1], out[-1][1])
+    for cv in (2, 0):
+        assert np.abs(out[cv][0] - out[1][0]).max() <= 1e-13 * np.abs(out[1][0]).max()
+    # theta_order 10 on a recompute-only handle uses the TMA column kernel (it reads that supply); without TMA it needs planes
+    g = teuk.Teuk.from_workload(w.scaled(dt_override=0.5 * w.dt), coef_variant=1)
+    g.set_option("theta_order", 10)
+    g.set_initial(u0)
+    g.step(3)
+    assert np.isfinite(g.read()).all()
+    g = teuk.Teuk.from_workload(w, coef_variant=1)
+    g.set_option("theta_order", 10)
+    g.set_option("use_tma", 0)
+    with pytest.raises(teuk.TeukError):
+        g.set_initial(u0)
