@@ -332,15 +332,18 @@ def run_sweep(args):
             for nt in (32, 64, 256):
                 w = workload(f"sweep:{nr}x{nt}:{L}")
                 steps = {1: 400, 2: 120, 4: 40}[L] if args.steps == 2000 else args.steps
-                r = time_device(torch, teuk, w, steps, 10, args.option, reps=3)
+                opts = list(args.option)
+                if L == 1 and not any(o.replace(" ", "").startswith("coef_variant") for o in opts):
+                    opts.append("coef_variant=1")      # explicit, so that the line is labelled with the supply that ran
+                r = time_device(torch, teuk, w, steps, 10, opts, reps=3)
                 ups = nr * nt * steps / (r["ms"] * 1e-3)
-                label, bpu = supply_of(args.option, L)
+                label, bpu = supply_of(opts, L)
                 line = {"workload": w.name, "precision_limbs": L, "n_r": nr, "n_theta": nt, "steps": steps,
                         "dt_over_dr": w.dt / w.dr, "updates_per_s": ups, "ms_per_step": r["ms"] / steps,
                         "ms_per_step_min": r["ms_min"] / steps, "finite": r["finite"], "geometry": r["geometry"],
                         "supply": label}
                 if L == 1:
-                    line["roofline"] = hbm_roofline(ups, nr * nt, bpu, peak, peak_src, kernel_name(L, args.option))
+                    line["roofline"] = hbm_roofline(ups, nr * nt, bpu, peak, peak_src, kernel_name(L, opts))
                     line["working_set_mib"] = int((bpu + 64) * nr * nt) // 2 ** 20
                 else:
                     line["roofline"] = pipe_roofline(ups, L, pipe, 10 if "theta_order=10" in args.option else 2)

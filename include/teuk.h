@@ -66,8 +66,9 @@ int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_the
 
 /* Options, only before teuk_set_initial (else TEUK_ESTATE): "graph_steps" (even, >= 2; steps per
  * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic), "use_tma" (fp64: 1 = TMA
- * kernel, default; 0 = generic kernel), "variant" (dd/qd launch shape 0..2), "coef_variant" (0 = precomputed
- * coefficient planes, default; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only -- the fastest fp64
+ * kernel, default; 0 = generic kernel), "variant" (dd/qd launch shape 0..2), "coef_variant" (default: automatic -- fp64 grids of >= 400 000 points step
+ * with variant 1, everything else and every run that sets one of the tile / time_block / theta_order / use_tma options with
+ * variant 0; 0 = precomputed coefficient planes; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only -- the fastest fp64
  * path (column-march kernel; "march" = 0 selects the older TMA tile kernel for the same supply, "march_chunk" = theta
  * rows per work unit, 0 = automatic); 2 = full recompute: 1-D tables only, 1/Sigma = rsqrt(R^2 - a^2 Delta sin^2 theta)
  * per point, fp64 only),

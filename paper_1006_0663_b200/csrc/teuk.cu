@@ -96,6 +96,7 @@ struct teuk_ctx {
     ThetaWeights tw;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
     bool use_tma = false, use_rc = false, use_col_tma = false, use_march = false;
+    int opt_cv = -1;                   // "coef_variant" option; -1 = automatic (resolved into coef_variant at teuk_set_initial)
     int opt_march = 1, opt_march_chunk = 0;   // fp64 semi-recompute supply: column-march kernel (step_kernel_march.cuh) unless march=0
     int march_strips = 0, march_chunk = 0, march_units = 0;
     CUtensorMap tm_state[2], tm_ch, tm_ci, tm_ish, tm_isi, tm_rth, tm_rti;
@@ -291,6 +292,7 @@ static int create_impl(double M, double a, int s, int m, int n_r_global, int i_l
     c->rmin = rstar_min; c->rmax = rstar_max; c->dt = dt; c->cap_alloc = obs_capacity;
     c->i_lo = i_lo; c->n_r_global = n_r_global;
     c->create_variant = cv; c->has_planes = cv_has_planes(precision, cv); c->has_rc = cv_has_rc(precision, cv);
+    c->opt_cv = cv;                    // a handle created for one supply uses it; -1: chosen at teuk_set_initial
     c->coef_variant = cv < 0 ? 0 : cv;
     c->ws = (char*)d_workspace; c->lay = lay; c->stream = (cudaStream_t)cuda_stream;
 
@@ -415,7 +417,7 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     } else if (!strcmp(key, "coef_variant")) {
         if (v < 0 || v > 2 || (v >= 1 && c->L != 1)) return TEUK_EINVAL;
         if (v == 0 ? !c->has_planes : !c->has_rc) return TEUK_EINVAL;      // that supply is not resident in this handle's workspace
-        c->coef_variant = v;
+        c->opt_cv = v;
     } else if (!strcmp(key, "variant")) {
         if (v < 0 || v > 2) return TEUK_EINVAL;
         c->variant = v;
@@ -579,7 +581,19 @@ static void fill_theta_weights(ThetaWeights& w) {
     for (int l = 0; l < 4; ++l) w.wd[0][l] = d0.x[l];
 }
 
+// fp64 grids from this many points on step faster with the semi-recompute column-march kernel than with the stored
+// planes (profiles/r02_sweep.md: 16384 x 32 and 4096 x 256 win, 4096 x 64 loses: too few work units for 1184 warps)
+constexpr long MARCH_AUTO_MIN_POINTS = 400000;
+
 static int choose_geometry(teuk_ctx* c) {
+    c->coef_variant = c->opt_cv;
+    if (c->opt_cv < 0) {
+        // automatic: the fastest parity-green supply for this grid, unless an option asks for a specific stored-plane kernel
+        const bool plain = c->theta_order == 2 && c->opt_tb == 1 && c->opt_tma && c->opt_march && c->opt_ti == 0 &&
+                           c->opt_tj == 0 && c->variant == 0;
+        const bool big = (long)c->n_r * c->n_theta >= MARCH_AUTO_MIN_POINTS && 4 * c->lay.plane < (1L << 31);
+        c->coef_variant = (c->L == 1 && c->has_rc && c->has_planes && plain && big) ? 1 : (c->has_planes ? 0 : 1);
+    }
     c->use_tma = false;
     c->use_rc = false;
     c->use_tb2 = false;
