@@ -257,14 +257,20 @@ def test_recomputed_coefficients_match_stored_planes(teuk, cfg):
         assert relc.max() <= 32 * 2.0 ** -52, (half, float(relc.max()), np.unravel_index(relc.argmax(), relc.shape))
 
 
-@pytest.mark.parametrize("n_r,n_t,base", [(203, 13, 2), (512, 16, 1), (1000, 70, 2), (40, 3, 2)])
-def test_recompute_kernel_parity_fp64(teuk, n_r, n_t, base):
-    w = inputs.config(base).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0)
+@pytest.mark.parametrize("n_r,n_t,base,m", [(203, 13, 2, 2), (512, 16, 1, 0), (1000, 70, 2, 2), (40, 3, 2, 2), (3, 2, 2, 1),
+                                             (31, 2, 2, 2), (61, 5, 2, 1), (32, 9, 2, 2), (30, 4, 2, 1)])
+def test_recompute_kernel_parity_fp64(teuk, n_r, n_t, base, m):
+    """semi-recompute supply on the column-march kernel (whole columns, automatic and odd work-unit lengths) and on the TMA
+    tile kernel, full recompute on the tile kernel; ragged and degenerate grids (3 columns, 2 rows, strips of exactly 30
+    and 30 + 1 + 1 columns), even and odd |m|"""
+    w = inputs.config(base).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0, m=m)
     w = w.scaled(dt_override=inputs.stable_dt(w))
     u0 = inputs.random_state(n_r, n_t, 1, seed=33)
     o = run_oracle(w, u0, 200, observer=(10.3, 1.1))
     ref, sref = o.read(), o.observe(200)
-    for opts in ({"coef_variant": 1}, {"coef_variant": 1, "tile_j": 8}, {"coef_variant": 2}, {"coef_variant": 2, "tile_j": 8}):
+    for opts in ({"coef_variant": 1}, {"coef_variant": 1, "march_chunk": n_t}, {"coef_variant": 1, "march_chunk": min(3, n_t)},
+                 {"coef_variant": 1, "march": 0}, {"coef_variant": 1, "march": 0, "tile_j": 8},
+                 {"coef_variant": 2}, {"coef_variant": 2, "tile_j": 8}):
         g = run_gpu(teuk, w, u0, 200, options=opts, observer=(10.3, 1.1))
         err = oracle.rel_linf(g.read(), ref)
         serr = series_err(g.observe(200), sref)
