@@ -15,7 +15,8 @@ prefix.  Stored per config:
     observer      [steps_done][4][L]   the observer series in full, all limbs
     checkpoints   [k]                  step counts at which the state was sampled (the last one = steps_done)
     state_<n>     [4][L][N_theta][n_cols]  every `stride`-th r* column of the state after n steps, all limbs
-                  (stride 8 at the last checkpoint of a completed run, 64 at the intermediate ones)
+                  (stride 8 at the last checkpoint of a completed run, 64 at the intermediate ones: 10 %, 20 %, 25 %, ...
+                  of the run; a run that was resumed under an older version of this script may lack some of them)
 """
 from __future__ import annotations
 
@@ -36,7 +37,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SOURCES = ["teuk_oracle.cpp", "mpx.hpp", "mpf.hpp", "mp_ref.py"]
 FINAL_STRIDE, MID_STRIDE = 8, 64
 # step counts at which the state is sampled (fractions of the run), the last one being the full length
-CHECKPOINT_FRACTIONS = (0.1, 0.25, 0.5, 0.75, 1.0)
+CHECKPOINT_FRACTIONS = (0.1, 0.2, 0.25, 0.3, 0.4, 0.5, 0.6, 0.7, 0.75, 0.8, 0.9, 1.0)
 
 
 def source_hash() -> str:
