@@ -64,20 +64,28 @@ int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_the
                      double dt, int precision, int coef_variant, int i_lo, int n_win, void *d_workspace,
                      size_t workspace_bytes, long obs_capacity, void *cuda_stream, teuk_ctx **out);
 
-/* Options, only before teuk_set_initial (else TEUK_ESTATE): "graph_steps" (even, >= 2; steps per
- * captured CUDA graph, default 32; 0 disables graphs), "tile_i", "tile_j" (0 = automatic), "use_tma" (fp64: 1 = TMA
- * kernel, default; 0 = generic kernel), "variant" (dd/qd launch shape 0..2), "coef_variant" (default: automatic -- fp64 grids of >= 400 000 points step
- * with variant 1, everything else and every run that sets one of the tile / time_block / theta_order / use_tma options with
- * variant 0; 0 = precomputed coefficient planes; 1 = semi-recompute supply: one 1/Sigma plane + 1-D tables, fp64 only -- the fastest fp64
- * path (column-march kernel; "march" = 0 selects the older TMA tile kernel for the same supply, "march_chunk" = theta
- * rows per work unit, 0 = automatic); 2 = full recompute: 1-D tables only, 1/Sigma = rsqrt(R^2 - a^2 Delta sin^2 theta)
- * per point, fp64 only),
- * "pdl" (fp64 TMA kernels: 1 = programmatic dependent launch, the next step prefetches its half-step coefficient
- * tile while the current one drains; default 0, measured neutral), "theta_order" (2 = second-order centred theta differences, default; 10 = the 10th-order
- * 11-point operator of PAPER.md:126, needs n_theta >= 5), "time_block" (1 = one iteration per launch, default; 2 = EXPERIMENT, two
- * iterations per launch on a shared-memory resident tile, fp64 stored-plane TMA path only, else TEUK_EINVAL at
- * teuk_set_initial; an odd last iteration and runs with the multipole observer use the one-iteration kernel; parity-green
- * but slower than coef_variant = 1, kept for the record). */
+/* Options, only before teuk_set_initial (else TEUK_ESTATE); unknown key or bad value: TEUK_EINVAL.
+ *  "graph_steps"   even, >= 2: iterations per captured CUDA graph (default 32); a teuk_step(n) call replays it n / 32
+ *                  times and runs the remainder as one more (cached) graph; 0 disables graphs.
+ *  "coef_variant"  coefficient supply (H1b).  Default: automatic -- fp64 grids of >= 400 000 points step with variant 1,
+ *                  everything else, and every run that sets tile_i / tile_j / use_tma / variant / time_block, with variant 0.
+ *                  0 = precomputed folded coefficient planes (192 L B of HBM traffic per update);
+ *                  1 = semi-recompute, fp64 only: one 1/Sigma plane per point family + 1-D tables, the eight coefficients
+ *                      are rebuilt in registers (80 B per update) -- the fastest fp64 path (column-march kernel);
+ *                  2 = full recompute, fp64 only: 1-D tables only, 1/Sigma = rsqrt(R^2 - a^2 Delta sin^2 theta) per point.
+ *                  A handle created for one supply (teuk_create's coef_variant >= 0) accepts only that one.
+ *  "march"         coef_variant 1: 1 = column-march kernel (default), 0 = the TMA tile kernel for the same supply.
+ *  "march_chunk"   column-march kernel: theta rows per work unit; 0 = chosen by the library (default).
+ *  "theta_order"   2 = second-order centred theta differences, PAPER.md:110 (default); 10 = the 10th-order 11-point
+ *                  operator of PAPER.md:126, needs n_theta >= 5.
+ *  "tile_i", "tile_j"  tile of the tile kernels; 0 = automatic (default).
+ *  "use_tma"       fp64: 1 = TMA kernels (default), 0 = the generic tile kernel.
+ *  "variant"       dd / qd launch shape 0..2 (0 = default).
+ *  "pdl"           fp64 TMA kernels: 1 = programmatic dependent launch (default 0; measured neutral).
+ *  "time_block"    1 = one iteration per launch (default); 2 = EXPERIMENT: two iterations per launch on a shared-memory
+ *                  resident tile, fp64 stored-plane TMA path only, else TEUK_EINVAL at teuk_set_initial; an odd last
+ *                  iteration and runs with the multipole observer use the one-iteration kernel.  Parity-green but slower
+ *                  than coef_variant = 1; kept for the record. */
 int teuk_set_option(teuk_ctx *, const char *key, double value);
 
 /* Observer at a fixed location: bilinear interpolation in (r*, theta) from the four
