@@ -308,7 +308,9 @@ def pipe_roofline(ups, L, pipe_peak, theta_order=2):
 def kernel_name(L, options):
     opt = {o.replace(" ", "") for o in options}
     if "theta_order=10" in opt:
-        return "step_kernel_f64_col_tma" if L == 1 else f"step_kernel_col<{L}>"
+        if L == 1:
+            return "step_kernel_col<1>" if "use_tma=0" in opt else ("step_kernel_f64_col_tma" if "col_run=0" in opt else "step_kernel_f64_col_run")
+        return f"step_kernel_col<{L}>"
     if L == 1:
         if "coef_variant=1" in opt:
             return "step_kernel_f64_rc" if "march=0" in opt else "step_kernel_f64_march"

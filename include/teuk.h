@@ -78,6 +78,8 @@ int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_the
  *  "march_chunk"   column-march kernel: theta rows per work unit; 0 = chosen by the library (default).
  *  "theta_order"   2 = second-order centred theta differences, PAPER.md:110 (default); 10 = the 10th-order 11-point
  *                  operator of PAPER.md:126, needs n_theta >= 5.
+ *  "col_run"       fp64, theta_order 10: 1 = a thread owns runs of 4 theta rows of a column (default), 0 = one point per
+ *                  thread (the round-1 kernel).
  *  "tile_i", "tile_j"  tile of the tile kernels; 0 = automatic (default).
  *  "use_tma"       fp64: 1 = TMA kernels (default), 0 = the generic tile kernel.
  *  "variant"       dd / qd launch shape 0..2 (0 = default).

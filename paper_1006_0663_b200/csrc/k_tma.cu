@@ -23,4 +23,10 @@ const void* col_tma_fn(int ti) {
     return nullptr;
 }
 
+const void* col_run_fn(int ti) {      // 256 threads, registers capped for 2 blocks per SM, runs of 4 rows
+    if (ti == 16) return (const void*)step_kernel_f64_col_run<16, 4, 256, 2>;
+    if (ti == 8) return (const void*)step_kernel_f64_col_run<8, 4, 256, 2>;
+    return nullptr;
+}
+
 }  // namespace tk

@@ -18,6 +18,7 @@ const void* generic_col_fn_4(int* threads);
 const void* tma_step_fn(int ti, int tj);
 const void* rc_step_fn(int ti, int tj, int full);     // full = H1b variant (c)
 const void* col_tma_fn(int ti);
+const void* col_run_fn(int ti);      // row-run variant (a thread owns 4 consecutive theta rows of a column), ti = 8 | 16
 // fp64 column-march kernel (step_kernel_march.cuh): semi-recompute supply, no shared-memory tiles
 const void* march_step_fn();
 // fp64 two-iterations-per-launch kernel (step_kernel_tb2.cuh, NEXT-3)

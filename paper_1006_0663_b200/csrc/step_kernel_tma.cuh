@@ -497,4 +497,182 @@ __global__ void __launch_bounds__(256) step_kernel_f64_col_tma(const __grid_cons
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// Row-run variant of the 10th-order fp64 column kernel (round 2).  Same tiles, same TMA loads and the same arithmetic
+// in the same order as step_kernel_f64_col_tma, but a thread owns a RUN of R consecutive theta rows of one column instead
+// of single points: the 11-point stencil's window of sig_Phi (R + 10 rows x 2 components) is loaded from shared memory once
+// per run and kept in registers (2 (R + 10) / R shared-memory loads per point instead of 22), and the 14 r-table entries of
+// the column are loaded once per run instead of once per point.  ncu on the point-per-thread kernel: 113 shared-memory
+// loads per update, shared-memory scoreboard 2.2-2.5 stalls per issued instruction.
+template <int TI, int R, int NTHR, int MINB>
+__global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __grid_constant__ CUtensorMap tm_u,
+                                                               const __grid_constant__ CUtensorMap tm_ish,
+                                                               const __grid_constant__ CUtensorMap tm_isi,
+                                                               const __grid_constant__ CUtensorMap tm_rth,
+                                                               const __grid_constant__ CUtensorMap tm_rti, StepParams P,
+                                                               RcParams Q, ThetaWeights W) {
+    using G = ColGeom<TI>;
+    constexpr int UC = G::UC, HC = G::HC, CC = G::CC, NT = G::NT, WIN = R + 10;
+    extern __shared__ __align__(128) unsigned char raw[];
+    __shared__ __align__(8) uint64_t bar[2];
+    const int nt = P.n_theta, nr = P.n_r;
+    auto a128 = [](size_t v) { return (v + 127) / 128 * 128; };
+    unsigned char* base = raw;
+    double* us = (double*)base;                      base += a128((size_t)4 * nt * UC * 8);
+    double* ish = (double*)base;                     base += a128((size_t)nt * CC * 8);
+    double* isi = (double*)base;                     base += a128((size_t)nt * TI * 8);
+    double* rth = (double*)base;                     base += a128((size_t)NT * CC * 8);
+    double* rti = (double*)base;                     base += a128((size_t)NT * TI * 8);
+    double* hs = (double*)base;                      base += a128((size_t)4 * nt * HC * 8);
+    double* ss = (double*)base;
+    const int i0 = blockIdx.x * TI;
+    const int tid = threadIdx.x;
+    const double sigma = P.sigma;
+
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&bar[0], (4 * nt * UC + nt * CC + NT * CC) * 8);
+        tma_load_3d(us, &tm_u, i0 - 2, 0, 0, &bar[0]);
+        tma_load_3d(ish, &tm_ish, i0 - 2, 0, 0, &bar[0]);
+        tma_load_3d(rth, &tm_rth, i0 - 2, 0, 0, &bar[0]);
+        mbar_expect_tx(&bar[1], (nt * TI + NT * TI) * 8);
+        tma_load_3d(isi, &tm_isi, i0, 0, 0, &bar[1]);
+        tma_load_3d(rti, &tm_rti, i0, 0, 0, &bar[1]);
+    }
+    mbar_wait(&bar[0], 0);
+
+    // sig_Phi = Phi(i+1) + Phi(i) at the TI+1 half points (u tile column of half point tc: tc+1 and tc+2)
+    for (int idx = tid; idx < 2 * nt * HC; idx += NTHR) {
+        int tc = idx % HC, rest = idx / HC;
+        ss[rest * HC + tc] = us[rest * UC + tc + 2] + us[rest * UC + tc + 1];
+    }
+    __syncthreads();
+
+    const int ngroups = (nt + R - 1) / R;
+    // the window of one component: rows j0-5 .. j0+R+4 of column `col` of a [2][nt][COLS] sig tile, polar ghosts mirrored
+    // with sign sigma (f_{-k} = sigma f_{k-1}, f_{N-1+k} = sigma f_{N-k})
+    auto load_window = [&](const double* tile, int cols, int col, int j0, double (&win)[2][WIN]) {
+#pragma unroll
+        for (int w = 0; w < WIN; ++w) {
+            int rr = j0 - 5 + w;
+            double sg = 1.0;
+            if (rr < 0) { rr = -rr - 1; sg = sigma; }
+            if (rr >= nt) { rr = 2 * nt - 1 - rr; sg = sigma; }
+            rr = min(max(rr, 0), nt - 1);                      // rows of a partial last run that nothing uses
+#pragma unroll
+            for (int c = 0; c < 2; ++c) win[c][w] = sg * tile[(c * nt + rr) * cols + col];
+        }
+    };
+    // Lambda at window position w (row j0 + w - 5 ... the centre is win[.][w]), same summation order as substep_wide
+    auto lam_at = [&](const double (&win)[2][WIN], int c, int w, double cj) {
+        double s2 = W.wd[0][0] * win[c][w];
+        double s1 = 0.0;
+#pragma unroll
+        for (int k = 1; k <= 5; ++k) {
+            const double up = win[c][w + k], dn = win[c][w - k];
+            s2 = s2 + W.wd[k][0] * (up + dn);
+            s1 = s1 + W.wc[k - 1][0] * (up - dn);
+        }
+        return s2 + cj * (s1 * 2.0);
+    };
+
+    // ---- half step, Eq. (13): tasks = (half-point column tc, run of R rows)
+    for (int task = tid; task < HC * ngroups; task += NTHR) {
+        const int g = task / HC, tc = task - g * HC, j0 = g * R;
+        const int ih = i0 - 1 + tc;
+        if (ih < 0 || ih > nr - 2) continue;
+        double win[2][WIN], rt[14];
+        load_window(ss, HC, tc, j0, win);
+#pragma unroll
+        for (int q = 0; q < 14; ++q) rt[q] = rth[q * CC + tc + 1];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int j = j0 + r;
+            if (j < nt) {
+                R1 sg[4], dl[4], lam[2], out[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const double lo = us[(c * nt + j) * UC + tc + 1], hi = us[(c * nt + j) * UC + tc + 2];
+                    sg[c].x[0] = (c < 2) ? win[c][r + 5] : hi + lo;
+                    dl[c].x[0] = hi - lo;
+                }
+                const double cj = __ldg(P.cj + j);
+#pragma unroll
+                for (int c = 0; c < 2; ++c) lam[c].x[0] = lam_at(win, c, r + 5, cj);
+                RcCoef cf;
+                rc_eval(cf, ish[j * CC + tc + 1], rt, 1, __ldg(Q.th + j), __ldg(Q.th + nt + j), __ldg(Q.th + 2 * nt + j));
+                substep_core<1, RTile<UC>, RcCoef>(sg, dl, lam, cf, P.tq_half, true, out, out);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) hs[(c * nt + j) * HC + tc] = out[c].x[0];
+            }
+        }
+    }
+    __syncthreads();
+    for (int idx = tid; idx < 2 * nt * TI; idx += NTHR) {      // sig_Phi of the half-step field, [2][nt][TI]
+        int tc = idx % TI, rest = idx / TI;
+        ss[rest * TI + tc] = hs[rest * HC + tc + 1] + hs[rest * HC + tc];
+    }
+    mbar_wait(&bar[1], 0);
+    __syncthreads();
+
+    // ---- full step, Eq. (14), radial Dirichlet columns, observer nodes: tasks = (output column tc, run of R rows)
+    for (int task = tid; task < TI * ngroups; task += NTHR) {
+        const int g = task / TI, tc = task - g * TI, j0 = g * R;
+        const int i = i0 + tc;
+        if (i >= nr) continue;
+        const bool wall = (i == 0 || i == nr - 1);
+        double win[2][WIN], rt[14];
+        load_window(ss, TI, tc, j0, win);
+#pragma unroll
+        for (int q = 0; q < 14; ++q) rt[q] = rti[q * TI + tc];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int j = j0 + r;
+            if (j < nt) {
+                R1 out[4];
+                if (wall) {
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) out[c].x[0] = 0.0;
+                } else {
+                    R1 sg[4], dl[4], lam[2], bs[4];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const double lo = hs[(c * nt + j) * HC + tc], hi = hs[(c * nt + j) * HC + tc + 1];
+                        sg[c].x[0] = (c < 2) ? win[c][r + 5] : hi + lo;
+                        dl[c].x[0] = hi - lo;
+                        bs[c].x[0] = us[(c * nt + j) * UC + tc + 2];
+                    }
+                    const double cj = __ldg(P.cj + j);
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) lam[c].x[0] = lam_at(win, c, r + 5, cj);
+                    RcCoef cf;
+                    rc_eval(cf, isi[j * TI + tc], rt, 1, __ldg(Q.th + j), __ldg(Q.th + nt + j), __ldg(Q.th + 2 * nt + j));
+                    substep_core<1, RTile<UC>, RcCoef>(sg, dl, lam, cf, P.tq_full, false, bs, out);
+                }
+                const long gidx = (long)j * P.pitch + i;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) P.u_out[(long)c * P.plane + gidx] = out[c].x[0];
+                if (P.obs_raw != nullptr) {
+                    const int di = i - P.oi, dj = j - P.oj;
+                    if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
+                        const long ks = *P.step_base + P.step_off;
+                        if (ks < P.obs_cap) {
+                            double* o = P.obs_raw + ((ks * 4 + (dj * 2 + di)) * 4);
+#pragma unroll
+                            for (int c = 0; c < 4; ++c) o[c] = out[c].x[0];
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
 }  // namespace tk

@@ -96,8 +96,9 @@ struct teuk_ctx {
     ThetaWeights tw;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
     bool use_tma = false, use_rc = false, use_col_tma = false, use_march = false;
+    const void* col_fn_ptr = nullptr;   // the fp64 10th-order TMA column kernel chosen by setup_col_tma
     int opt_cv = -1;                   // "coef_variant" option; -1 = automatic (resolved into coef_variant at teuk_set_initial)
-    int opt_march = 1, opt_march_chunk = 0;   // fp64 semi-recompute supply: column-march kernel (step_kernel_march.cuh) unless march=0
+    int opt_march = 1, opt_march_chunk = 0, opt_col_run = 1;   // fp64 semi-recompute supply: column-march kernel (step_kernel_march.cuh) unless march=0
     int march_strips = 0, march_chunk = 0, march_units = 0;
     CUtensorMap tm_state[2], tm_ch, tm_ci, tm_ish, tm_isi, tm_rth, tm_rti;
     // temporally blocked fp64 path (two iterations per launch, step_kernel_tb2.cuh): its own boxes, grid and smem
@@ -424,6 +425,8 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
     } else if (!strcmp(key, "time_block")) {
         if ((v != 1 && v != 2) || (v == 2 && c->L != 1)) return TEUK_EINVAL;
         c->opt_tb = v;
+    } else if (!strcmp(key, "col_run")) {
+        c->opt_col_run = v != 0;
     } else if (!strcmp(key, "march")) {
         c->opt_march = v != 0;
     } else if (!strcmp(key, "march_chunk")) {        // theta rows per work unit of the march kernel (0 = chosen by the library)
@@ -538,7 +541,7 @@ template <int TI, int TJ> static bool setup_rc(teuk_ctx* c) {
     return true;
 }
 
-template <int TI> static bool setup_col_tma(teuk_ctx* c) {
+template <int TI> static bool setup_col_tma(teuk_ctx* c, bool row_run) {
     using G = ColGeom<TI>;
     const Layout& y = c->lay;
     const int nt = c->n_theta;
@@ -552,9 +555,10 @@ template <int TI> static bool setup_col_tma(teuk_ctx* c) {
               make_map(&c->tm_rth, rt0 + (size_t)RC_NT * y.pitch, c->n_r - 1, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, G::CC, RC_NT, 1);
     size_t sm = G::total(nt);
     if (!ok || sm > 227 * 1024) return false;
-    const void* fn = col_tma_fn(TI);
+    const int threads = 256;
+    const void* fn = row_run ? col_run_fn(TI) : col_tma_fn(TI);
     if (!fn || cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess) return false;
-    c->ti = TI; c->tj = nt; c->smem = sm; c->threads = 256;
+    c->ti = TI; c->tj = nt; c->smem = sm; c->threads = threads; c->col_fn_ptr = fn;
     c->grid = dim3((c->n_r + TI - 1) / TI, 1);
     return true;
 }
@@ -606,7 +610,10 @@ static int choose_geometry(teuk_ctx* c) {
             // automatic tile: 16 columns when N_theta <= 64 (half the block barriers and one redundant half-step column per
             // 16 instead of per 8: measured 3-5 % faster on 16384 x 64 and 65536 x 64 although one block per SM), else 8
             const int ti = c->opt_ti ? c->opt_ti : (c->n_theta <= 64 && c->n_r >= 2048 ? 16 : 8);
-            bool ok = ti == 16 ? setup_col_tma<16>(c) : ti == 12 ? setup_col_tma<12>(c) : setup_col_tma<8>(c);
+            // kernel: row runs (a thread owns 4 consecutive rows of a column, stencil window in registers; +22 % on
+            // config 2) unless "col_run" = 0 or the 12-column tile is asked for: then one point per thread
+            const bool rr = c->opt_col_run && ti != 12;
+            bool ok = ti == 16 ? setup_col_tma<16>(c, rr) : ti == 12 ? setup_col_tma<12>(c, false) : setup_col_tma<8>(c, rr);
             cudaGetLastError();
             if (ok) { c->use_col_tma = true; return TEUK_OK; }
         }
@@ -727,7 +734,7 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
     if (c->theta_order == 10 && c->use_col_tma) {
         RcParams Q{c->dptr(c->lay.rc_th)};
         void* args[] = {&c->tm_state[from], &c->tm_ish, &c->tm_isi, &c->tm_rth, &c->tm_rti, &P, &Q, &c->tw};
-        if (cudaLaunchKernel(col_tma_fn(c->ti), c->grid, dim3(256), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
+        if (cudaLaunchKernel(c->col_fn_ptr, c->grid, dim3(c->threads), args, c->smem, c->stream) != cudaSuccess) return TEUK_ECUDA;
     } else if (c->theta_order == 10) {
         void* args[] = {&P, &c->tw};
         int threads = 256;

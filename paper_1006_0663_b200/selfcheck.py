@@ -44,7 +44,8 @@ def main() -> int:
         ("two iterations per launch (step2_kernel_f64_tma)", 1, {"time_block": 2}),
         ("double-double (step_kernel<2>)", 2, {}),
         ("quad-double (step_kernel<4>)", 4, {}),
-        ("theta order 10, fp64 TMA columns (step_kernel_f64_col_tma)", 1, {"theta_order": 10}),
+        ("theta order 10, fp64 TMA columns, row runs (step_kernel_f64_col_run)", 1, {"theta_order": 10}),
+        ("theta order 10, fp64 TMA columns, point per thread (step_kernel_f64_col_tma)", 1, {"theta_order": 10, "col_run": 0}),
         ("theta order 10, fp64 generic columns (step_kernel_col<1>)", 1, {"theta_order": 10, "use_tma": 0}),
         ("theta order 10, double-double (step_kernel_col<2>)", 2, {"theta_order": 10}),
         ("theta order 10, quad-double (step_kernel_col<4>)", 4, {"theta_order": 10}),

@@ -20,7 +20,9 @@ FAMILIES = [
     ("f64_tb2", 1, {"time_block": 2}),
     ("dd", 2, {}),
     ("qd", 4, {}),
-    ("f64_col_tma", 1, {"theta_order": 10}),
+    ("f64_col_run", 1, {"theta_order": 10}),
+    ("f64_col_run8", 1, {"theta_order": 10, "tile_i": 8}),
+    ("f64_col_tma", 1, {"theta_order": 10, "col_run": 0}),
     ("f64_col", 1, {"theta_order": 10, "use_tma": 0}),
     ("dd_col", 2, {"theta_order": 10}),
     ("qd_col", 4, {"theta_order": 10}),

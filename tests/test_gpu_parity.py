@@ -316,11 +316,12 @@ def test_theta10_parity_all_precisions(teuk, L, n_r, n_t, steps, base):
     assert not np.array_equal(g2.read(), g.read())
 
 
-@pytest.mark.parametrize("n_r,n_t", [(203, 13), (300, 64), (64, 5), (1000, 70)])
-def test_theta10_fp64_tma_column_kernel(teuk, n_r, n_t):
-    """fp64 theta_order=10 defaults to the TMA column kernel (semi-recompute supply); all its tile widths and the
-    generic column kernel must agree with the oracle"""
-    w = inputs.config(2).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0)
+@pytest.mark.parametrize("n_r,n_t,m", [(203, 13, 2), (300, 64, 2), (64, 5, 1), (1000, 70, 2), (2100, 30, 1), (40, 6, 2), (17, 9, 1)])
+def test_theta10_fp64_tma_column_kernel(teuk, n_r, n_t, m):
+    """fp64 theta_order=10 defaults to the TMA column kernels (semi-recompute supply): the row-run kernel (8- and 16-column
+    tiles; N_theta not a multiple of the run length, runs that straddle both poles, odd |m|), the point-per-thread kernel
+    at all its tile widths and the generic column kernel must agree with the oracle"""
+    w = inputs.config(2).scaled(n_r=n_r, n_theta=n_t, rstar_min=-30.0, rstar_max=60.0, m=m)
     w = w.scaled(dt_override=0.5 * inputs.stable_dt(w))
     u0 = inputs.random_state(n_r, n_t, 1, seed=77)
     o = oracle.Oracle.from_workload(w, theta_order=10)
@@ -328,7 +329,8 @@ def test_theta10_fp64_tma_column_kernel(teuk, n_r, n_t):
     o.set_initial(u0)
     o.step(80)
     ref, sref = o.read(), o.observe(80)
-    for opts in ({}, {"tile_i": 12}, {"tile_i": 16}, {"use_tma": 0}):
+    for opts in ({}, {"tile_i": 8}, {"tile_i": 16}, {"col_run": 0}, {"col_run": 0, "tile_i": 8}, {"tile_i": 12},
+                 {"col_run": 0, "tile_i": 16}, {"use_tma": 0}):
         g = run_gpu(teuk, w, u0, 80, observer=(10.3, 1.1), options={"theta_order": 10, **opts})
         geom = g.step_geometry()
         assert geom["tile_j"] == n_t
