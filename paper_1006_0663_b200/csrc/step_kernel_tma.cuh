@@ -13,6 +13,7 @@
 #include <cuda.h>
 
 #include <cstdint>
+#include <type_traits>
 
 #include "step_kernel.cuh"
 
@@ -558,9 +559,10 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
     const int ngroups = (nt + R - 1) / R;
     // the window of one component: rows j0-5 .. j0+R+4 of column `col` of a [2][nt][COLS] sig tile, polar ghosts mirrored
     // with sign sigma (f_{-k} = sigma f_{k-1}, f_{N-1+k} = sigma f_{N-k})
-    auto load_window = [&](const double* tile, int cols, int col, int j0, double (&win)[2][WIN]) {
+    auto load_window = [&](const double* tile, int cols, int col, int j0, auto& win) {
+        constexpr int WN = sizeof(win[0]) / sizeof(double);
 #pragma unroll
-        for (int w = 0; w < WIN; ++w) {
+        for (int w = 0; w < WN; ++w) {
             int rr = j0 - 5 + w;
             double sg = 1.0;
             if (rr < 0) { rr = -rr - 1; sg = sigma; }
@@ -571,7 +573,7 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
         }
     };
     // Lambda at window position w (row j0 + w - 5 ... the centre is win[.][w]), same summation order as substep_wide
-    auto lam_at = [&](const double (&win)[2][WIN], int c, int w, double cj) {
+    auto lam_at = [&](const auto& win, int c, int w, double cj) {
         double s2 = W.wd[0][0] * win[c][w];
         double s1 = 0.0;
 #pragma unroll
@@ -583,17 +585,17 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
         return s2 + cj * (s1 * 2.0);
     };
 
-    // ---- half step, Eq. (13): tasks = (half-point column tc, run of R rows)
-    for (int task = tid; task < HC * ngroups; task += NTHR) {
-        const int g = task / HC, tc = task - g * HC, j0 = g * R;
+    // ---- half step, Eq. (13): a task = (half-point column tc, run of RR rows starting at j0)
+    auto half_task = [&](auto RRc, int tc, int j0) {
+        constexpr int RR = decltype(RRc)::value;
         const int ih = i0 - 1 + tc;
-        if (ih < 0 || ih > nr - 2) continue;
-        double win[2][WIN], rt[14];
+        if (ih < 0 || ih > nr - 2) return;
+        double win[2][RR + 10], rt[14];
         load_window(ss, HC, tc, j0, win);
 #pragma unroll
         for (int q = 0; q < 14; ++q) rt[q] = rth[q * CC + tc + 1];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
+        for (int r = 0; r < RR; ++r) {
             const int j = j0 + r;
             if (j < nt) {
                 R1 sg[4], dl[4], lam[2], out[4];
@@ -613,6 +615,17 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
                 for (int c = 0; c < 4; ++c) hs[(c * nt + j) * HC + tc] = out[c].x[0];
             }
         }
+    };
+    // as many columns as one pass of the block covers go in runs of R rows; the columns that would need a second pass
+    // (the 17th half-step column of a 16-column tile at N_theta = 64) go row by row, spread over the threads again
+    const int main_cols = (ngroups <= NTHR) ? min(HC, NTHR / ngroups) : 0;
+    for (int task = tid; task < main_cols * ngroups; task += NTHR) {
+        const int g = task / main_cols, tc = task - g * main_cols;
+        half_task(std::integral_constant<int, R>{}, tc, g * R);
+    }
+    for (int task = tid; task < (HC - main_cols) * nt; task += NTHR) {
+        const int j = task / (HC - main_cols), tc = main_cols + task - j * (HC - main_cols);
+        half_task(std::integral_constant<int, 1>{}, tc, j);
     }
     __syncthreads();
     for (int idx = tid; idx < 2 * nt * TI; idx += NTHR) {      // sig_Phi of the half-step field, [2][nt][TI]
