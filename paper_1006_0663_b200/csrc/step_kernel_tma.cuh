@@ -388,6 +388,10 @@ template <int TI> struct ColGeom {
         return a128((size_t)4 * nt * UC * 8) + a128((size_t)nt * CC * 8) + a128((size_t)nt * TI * 8) + a128((size_t)NT * CC * 8) +
                a128((size_t)NT * TI * 8) + a128((size_t)4 * nt * HC * 8) + a128((size_t)2 * nt * HC * 8) + 128;
     }
+    static size_t total_run(int nt) {          // row-run kernel: no staged sig tile, + the four theta tables
+        return a128((size_t)4 * nt * UC * 8) + a128((size_t)nt * CC * 8) + a128((size_t)nt * TI * 8) + a128((size_t)NT * CC * 8) +
+               a128((size_t)NT * TI * 8) + a128((size_t)4 * nt * HC * 8) + a128((size_t)4 * nt * 8) + 128;
+    }
 };
 
 template <int TI>
@@ -526,7 +530,7 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
     double* rth = (double*)base;                     base += a128((size_t)NT * CC * 8);
     double* rti = (double*)base;                     base += a128((size_t)NT * TI * 8);
     double* hs = (double*)base;                      base += a128((size_t)4 * nt * HC * 8);
-    double* ss = (double*)base;
+    double* tht = (double*)base;                     // [4][nt]: cj, sin^2, cos, Tth
     const int i0 = blockIdx.x * TI;
     const int tid = threadIdx.x;
     const double sigma = P.sigma;
@@ -547,14 +551,11 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
         tma_load_3d(isi, &tm_isi, i0, 0, 0, &bar[1]);
         tma_load_3d(rti, &tm_rti, i0, 0, 0, &bar[1]);
     }
+    for (int k = tid; k < 4 * nt; k += NTHR) tht[k] = (k < nt) ? __ldg(P.cj + k) : __ldg(Q.th + (k - nt));
+    __syncthreads();
     mbar_wait(&bar[0], 0);
 
-    // sig_Phi = Phi(i+1) + Phi(i) at the TI+1 half points (u tile column of half point tc: tc+1 and tc+2)
-    for (int idx = tid; idx < 2 * nt * HC; idx += NTHR) {
-        int tc = idx % HC, rest = idx / HC;
-        ss[rest * HC + tc] = us[rest * UC + tc + 2] + us[rest * UC + tc + 1];
-    }
-    __syncthreads();
+    // sig_Phi = Phi(i+1) + Phi(i) is formed on the fly while a run's window is loaded (no staging pass, no barrier)
 
     const int ngroups = (nt + R - 1) / R;
     // the window of one component: rows j0-5 .. j0+R+4 of column `col` of a [2][nt][COLS] sig tile, polar ghosts mirrored
@@ -569,7 +570,7 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
             if (rr >= nt) { rr = 2 * nt - 1 - rr; sg = sigma; }
             rr = min(max(rr, 0), nt - 1);                      // rows of a partial last run that nothing uses
 #pragma unroll
-            for (int c = 0; c < 2; ++c) win[c][w] = sg * tile[(c * nt + rr) * cols + col];
+            for (int c = 0; c < 2; ++c) win[c][w] = sg * (tile[(c * nt + rr) * cols + col + 1] + tile[(c * nt + rr) * cols + col]);
         }
     };
     // Lambda at window position w (row j0 + w - 5 ... the centre is win[.][w]), same summation order as substep_wide
@@ -591,7 +592,7 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
         const int ih = i0 - 1 + tc;
         if (ih < 0 || ih > nr - 2) return;
         double win[2][RR + 10], rt[14];
-        load_window(ss, HC, tc, j0, win);
+        load_window(us, UC, tc + 1, j0, win);
 #pragma unroll
         for (int q = 0; q < 14; ++q) rt[q] = rth[q * CC + tc + 1];
 #pragma unroll
@@ -605,11 +606,11 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
                     sg[c].x[0] = (c < 2) ? win[c][r + 5] : hi + lo;
                     dl[c].x[0] = hi - lo;
                 }
-                const double cj = __ldg(P.cj + j);
+                const double cj = tht[j];
 #pragma unroll
                 for (int c = 0; c < 2; ++c) lam[c].x[0] = lam_at(win, c, r + 5, cj);
                 RcCoef cf;
-                rc_eval(cf, ish[j * CC + tc + 1], rt, 1, __ldg(Q.th + j), __ldg(Q.th + nt + j), __ldg(Q.th + 2 * nt + j));
+                rc_eval(cf, ish[j * CC + tc + 1], rt, 1, tht[nt + j], tht[2 * nt + j], tht[3 * nt + j]);
                 substep_core<1, RTile<UC>, RcCoef>(sg, dl, lam, cf, P.tq_half, true, out, out);
 #pragma unroll
                 for (int c = 0; c < 4; ++c) hs[(c * nt + j) * HC + tc] = out[c].x[0];
@@ -627,11 +628,6 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
         const int j = task / (HC - main_cols), tc = main_cols + task - j * (HC - main_cols);
         half_task(std::integral_constant<int, 1>{}, tc, j);
     }
-    __syncthreads();
-    for (int idx = tid; idx < 2 * nt * TI; idx += NTHR) {      // sig_Phi of the half-step field, [2][nt][TI]
-        int tc = idx % TI, rest = idx / TI;
-        ss[rest * TI + tc] = hs[rest * HC + tc + 1] + hs[rest * HC + tc];
-    }
     mbar_wait(&bar[1], 0);
     __syncthreads();
 
@@ -642,7 +638,7 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
         if (i >= nr) continue;
         const bool wall = (i == 0 || i == nr - 1);
         double win[2][WIN], rt[14];
-        load_window(ss, TI, tc, j0, win);
+        load_window(hs, HC, tc, j0, win);
 #pragma unroll
         for (int q = 0; q < 14; ++q) rt[q] = rti[q * TI + tc];
 #pragma unroll
@@ -662,11 +658,11 @@ __global__ void __launch_bounds__(NTHR, MINB) step_kernel_f64_col_run(const __gr
                         dl[c].x[0] = hi - lo;
                         bs[c].x[0] = us[(c * nt + j) * UC + tc + 2];
                     }
-                    const double cj = __ldg(P.cj + j);
+                    const double cj = tht[j];
 #pragma unroll
                     for (int c = 0; c < 2; ++c) lam[c].x[0] = lam_at(win, c, r + 5, cj);
                     RcCoef cf;
-                    rc_eval(cf, isi[j * TI + tc], rt, 1, __ldg(Q.th + j), __ldg(Q.th + nt + j), __ldg(Q.th + 2 * nt + j));
+                    rc_eval(cf, isi[j * TI + tc], rt, 1, tht[nt + j], tht[2 * nt + j], tht[3 * nt + j]);
                     substep_core<1, RTile<UC>, RcCoef>(sg, dl, lam, cf, P.tq_full, false, bs, out);
                 }
                 const long gidx = (long)j * P.pitch + i;

@@ -553,7 +553,7 @@ template <int TI> static bool setup_col_tma(teuk_ctx* c, bool row_run) {
               make_map(&c->tm_ish, is0 + y.plane, c->n_r - 1, nt, 1, y.pitch, y.plane, G::CC, nt, 1) &&
               make_map(&c->tm_rti, rt0, c->n_r, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, TI, RC_NT, 1) &&
               make_map(&c->tm_rth, rt0 + (size_t)RC_NT * y.pitch, c->n_r - 1, RC_NT, 1, y.pitch, (long)RC_NT * y.pitch, G::CC, RC_NT, 1);
-    size_t sm = G::total(nt);
+    size_t sm = row_run ? G::total_run(nt) : G::total(nt);
     if (!ok || sm > 227 * 1024) return false;
     const int threads = 256;
     const void* fn = row_run ? col_run_fn(TI) : col_tma_fn(TI);
