@@ -13,6 +13,7 @@
 //   new_Pi  = base_Pi  + c0 del_Pi  + [ -(c1 + i c2) sig_Pi + (c3 + i c4) del_Phi + c7 Lam - (c5 + i c6) sig_Phi ]
 // base = sig/2 for the half step, u^n for the full step.  Multiplications by 1/2 and 2 are exact.
 #pragma once
+#include <cstdint>
 #include "mp.cuh"
 
 namespace tk {
@@ -34,6 +35,16 @@ struct StepParams {
     int step_off;
     int oi, oj;              // lower-left observer node
 };
+
+// 8-byte asynchronous global -> shared copy; ok = false copies nothing and writes zeros (src-size 0), so lanes whose
+// column lies outside the grid take the same instruction as everyone else
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc, bool ok) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc),
+                 "r"(ok ? 8 : 0)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <int L> struct Ld {
     static __device__ __forceinline__ Real<L> g(const double* __restrict__ p, long stride, long idx) {
@@ -250,28 +261,20 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel(StepParams P) {
     bool v = item1(idx, tc, tr, gi, gj);
     if (PF && v) load_coef(cc, P.coef_h, P.plane, (long)gj * P.pitch + gi);
 
-    // ---- phase 0: stage the u^n tile (+1 column, +2 rows of halo); outside the grid -> 0
-    //      (loads issued in batches of STG before any of them is stored: one round trip to L2/HBM per batch instead of
-    //      one per element - the unbatched loop was the largest long-scoreboard stall of the dd kernel)
-    constexpr int STG = 8;
+    // ---- phase 0: stage the u^n tile (+1 column, +2 rows of halo); outside the grid -> 0.
+    //      8-byte cp.async with zero-fill: every element of the tile is in flight at once (ONE round trip to L2/HBM per
+    //      block, no staging registers); the register-batched loop this replaces took ceil(n_stage / (8 nth)) = 3 (dd)
+    //      or 4 (qd) dependent round trips, during which the block's warps left the FP64 pipe idle
     const int n_stage = 4 * L * UR * UC;
-    for (int k0 = tid; k0 < n_stage; k0 += nth * STG) {
-        double vals[STG];
-#pragma unroll
-        for (int u = 0; u < STG; ++u) {
-            int k = k0 + u * nth;
-            int c = k % UC, rest = k / UC;
-            int r = rest % UR, pl = rest / UR;
-            int ui = iu0 + c, uj = ju0 + r;
-            vals[u] = (k < n_stage && ui >= 0 && ui < nr && uj >= 0 && uj < nt)
-                          ? __ldg(P.u_in + pl * P.plane + (long)uj * P.pitch + ui) : 0.0;
-        }
-#pragma unroll
-        for (int u = 0; u < STG; ++u) {
-            int k = k0 + u * nth;
-            if (k < n_stage) us[k] = vals[u];
-        }
+    for (int k = tid; k < n_stage; k += nth) {
+        int c = k % UC, rest = k / UC;
+        int r = rest % UR, pl = rest / UR;
+        int ui = iu0 + c, uj = ju0 + r;
+        bool ok = ui >= 0 && ui < nr && uj >= 0 && uj < nt;
+        cp_async8(us + k, ok ? P.u_in + pl * P.plane + (long)uj * P.pitch + ui : P.u_in, ok);
     }
+    cp_async_commit();
+    cp_async_wait<0>();
     __syncthreads();
 
     SmemTile<L> ut{us, UR, UC, ju0};

@@ -72,15 +72,7 @@ constexpr int MARCH_RING = 16;      // rows resident per warp (power of two: slo
 constexpr int MARCH_PF = 11;        // rows requested ahead of the one being consumed (stage C still reads row r - 4)
 constexpr int MARCH_ROW = 6 * 32;   // doubles per ring row
 
-// 8-byte asynchronous global -> shared copy; ok = false copies nothing and writes zeros (src-size 0), so lanes whose
-// column lies outside the grid take the same instruction as everyone else
-__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc, bool ok) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc),
-                 "r"(ok ? 8 : 0)
-                 : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+// (cp_async8 / cp_async_commit / cp_async_wait: step_kernel.cuh)
 
 constexpr size_t march_smem_bytes(int n_theta) {
     return ((size_t)4 * n_theta + (size_t)MARCH_WARPS * MARCH_RING * MARCH_ROW + 8) * sizeof(double);
