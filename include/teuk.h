@@ -82,7 +82,10 @@ int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_the
  *                  thread (the round-1 kernel).
  *  "tile_i", "tile_j"  tile of the tile kernels; 0 = automatic (default).
  *  "use_tma"       fp64: 1 = TMA kernels (default), 0 = the generic tile kernel.
- *  "variant"       dd / qd launch shape 0..2 (0 = default).
+ *  "variant"       dd / qd kernel and launch shape: 0 = default (dd: one thread per point, 32 x 16 tile; qd: the pair
+ *                  kernel, two threads per point, 16 x 16 tile); 1, 2 = one thread per point with other launch bounds;
+ *                  3 = pair kernel (dd 32 x 16; qd 16 x 16, 32 x 8 or 16 x 8 by tile_i / tile_j); 4 = qd one thread per
+ *                  point on its 16 x 8 tile (the default before the pair kernel).  All bitwise identical in result.
  *  "pdl"           fp64 TMA kernels: 1 = programmatic dependent launch (default 0; measured neutral).
  *  "time_block"    1 = one iteration per launch (default); 2 = EXPERIMENT: two iterations per launch on a shared-memory
  *                  resident tile, fp64 stored-plane TMA path only, else TEUK_EINVAL at teuk_set_initial; an odd last

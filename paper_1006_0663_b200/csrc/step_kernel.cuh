@@ -360,6 +360,147 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel(StepParams P) {
 
 
 // ---------------------------------------------------------------------------------------------------------------
+// Pair kernel (dd / qd): TWO threads per point.  Lanes 2k and 2k+1 of a warp own the real and the imaginary part of
+// one point: lane part p computes Phi component p and Pi component 2+p.  Every sum / difference of the two radial
+// neighbours is formed once, by the lane that owns the component, and the three the OTHER part needs (sig of the
+// other Phi and Pi component, del of the other Phi component) travel by __shfl_xor, so the FP64 work per point is
+// exactly step_kernel's, operation for operation (sub(a, b) = add(a, neg(b)) and the +-1 factors are exact: results
+// are bitwise those of step_kernel).  Why: the straight-line qd sub-step is ~100 KB of code per phase and each warp
+// walks it once per point - ncu attributes 24 % of the qd kernel's stall samples to instruction fetch ("no_instruction");
+// here the body is half as long, each thread needs half the live values (more resident warps), and a warp covers 16
+// points per pass of the code.  Compile-time tile only.
+template <int L> __device__ __forceinline__ Real<L> partner(const Real<L>& a, unsigned mask) {
+    Real<L> r;
+#pragma unroll
+    for (int l = 0; l < L; ++l) r.x[l] = __shfl_xor_sync(mask, a.x[l], 1);
+    return r;
+}
+
+// one sub-step for part p of one point; t: tile accessor; cf/stride/idx: the point's 8 folded coefficients in global memory
+template <int L, class Tile>
+__device__ __forceinline__ void substep_pair(const Tile& t, int p, double sx, unsigned mask, int row, int rm, int rp, double sm,
+                                             double sp, int clo, int chi, const double* __restrict__ cf, long stride, long idx,
+                                             const Real<L>& cjv, double tq, bool half, const Real<L>& baseP, const Real<L>& basePi,
+                                             Real<L>& outP, Real<L>& outPi) {
+    const int cP = p, cPi = 2 + p;
+    GlobalCoef<L> g{cf, stride, idx};
+    Real<L> lo = t.get(cP, row, clo), hi = t.get(cP, row, chi);
+    const Real<L> sgP = add(hi, lo), dlP = sub(hi, lo);
+    lo = t.get(cPi, row, clo); hi = t.get(cPi, row, chi);
+    const Real<L> sgPi = add(hi, lo), dlPi = sub(hi, lo);
+    const Real<L> sgQ = partner(sgP, mask), dlQ = partner(dlP, mask), sgQi = partner(sgPi, mask);
+    // angular operator on this part's sig_Phi
+    const Real<L> up = sgn(add(t.get(cP, rp, chi), t.get(cP, rp, clo)), sp);
+    const Real<L> dn = sgn(add(t.get(cP, rm, chi), t.get(cP, rm, clo)), sm);
+    const Real<L> second = sub(add(up, dn), scale2(sgP, 2.0));
+    const Real<L> first = mul(cjv, sub(up, dn));
+    const Real<L> lam = add(second, first);
+    // tau * S_Pi for this part, in substep_core's order; sx = -1 (real part) / +1 (imaginary part) on the cross terms
+    Real<L> s = neg(add(mul(g.get(1), sgPi), sgn(mul(g.get(2), sgQi), sx)));
+    s = add(s, add(mul(g.get(3), dlP), sgn(mul(g.get(4), dlQ), sx)));
+    s = add(s, mul(g.get(7), lam));
+    s = sub(s, add(mul(g.get(5), sgP), sgn(mul(g.get(6), sgQ), sx)));
+    const Real<L> c0 = g.get(0);
+    const Real<L> bP = half ? scale2(sgP, 0.5) : baseP;
+    const Real<L> bPi = half ? scale2(sgPi, 0.5) : basePi;
+    outP = add(sub(bP, mul(c0, dlP)), mul_d(sgPi, tq));
+    outPi = add(add(bPi, mul(c0, dlPi)), s);
+}
+
+template <int L, int TI, int TJ, int NTHR, int MINB>
+__global__ void __launch_bounds__(NTHR, MINB) step_kernel_pair(StepParams P) {
+    static_assert(NTHR % 64 == 0, "two lanes per point, whole warps");
+    extern __shared__ double smem[];
+    constexpr int UC = TI + 2, UR = TJ + 4, HC = TI + 1, HR = TJ + 2, NP = NTHR / 2;
+    double* us = smem;                       // [4L][UR][UC]
+    double* hs = smem + 4 * L * UR * UC;     // [4L][HR][HC]
+    const int i0 = blockIdx.x * TI, j0 = blockIdx.y * TJ;
+    const int iu0 = i0 - 1, ju0 = j0 - 2, jh0 = j0 - 1;
+    const int nt = P.n_theta, nr = P.n_r;
+    const int tid = threadIdx.x;
+    const int p = tid & 1, cP = p, cPi = 2 + p;
+    const double sx = p ? 1.0 : -1.0;
+
+    // ---- phase 0: the u^n tile, as in step_kernel
+    constexpr int n_stage = 4 * L * UR * UC;
+    for (int k = tid; k < n_stage; k += NTHR) {
+        int c = k % UC, rest = k / UC;
+        int r = rest % UR, pl = rest / UR;
+        int ui = iu0 + c, uj = ju0 + r;
+        bool ok = ui >= 0 && ui < nr && uj >= 0 && uj < nt;
+        cp_async8(us + k, ok ? P.u_in + pl * P.plane + (long)uj * P.pitch + ui : P.u_in, ok);
+    }
+    cp_async_commit();
+    cp_async_wait<0>();
+    __syncthreads();
+
+    SmemTile<L> ut{us, UR, UC, ju0};
+    // ---- phase 1: half step, Eq. (13)
+    for (int q0 = 0; q0 < HR * HC; q0 += NP) {
+        const int q = q0 + (tid >> 1);
+        const int tr = q / HC, tc = q - tr * HC;
+        const int ih = iu0 + tc, jh = jh0 + tr;
+        const bool v = q < HR * HC && ih >= 0 && ih <= nr - 2 && jh >= 0 && jh < nt;
+        const unsigned mask = __ballot_sync(0xffffffffu, v);
+        if (v) {
+            int rm = jh - 1, rp = jh + 1;
+            double sm = 1.0, sp = 1.0;
+            if (rm < 0) { rm = 0; sm = P.sigma; }
+            if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+            Real<L> cjv = Ld<L>::g(P.cj, nt, jh);
+            Real<L> oP, oPi;
+            substep_pair<L>(ut, p, sx, mask, jh, rm, rp, sm, sp, tc, tc + 1, P.coef_h, P.plane, (long)jh * P.pitch + ih, cjv,
+                            P.tq_half, true, oP, oPi, oP, oPi);
+#pragma unroll
+            for (int l = 0; l < L; ++l) {
+                hs[(cP * L + l) * HR * HC + tr * HC + tc] = oP.x[l];
+                hs[(cPi * L + l) * HR * HC + tr * HC + tc] = oPi.x[l];
+            }
+        }
+    }
+    __syncthreads();
+
+    SmemTile<L> ht{hs, HR, HC, jh0};
+    // ---- phase 2: full step, Eq. (14), + radial Dirichlet rows + observer nodes
+    for (int q0 = 0; q0 < TJ * TI; q0 += NP) {
+        const int q = q0 + (tid >> 1);
+        const int tr = q / TI, tc = q - tr * TI;
+        const int i = i0 + tc, j = j0 + tr;
+        const bool v = q < TJ * TI && i < nr && j < nt;
+        const bool interior = v && i != 0 && i != nr - 1;
+        const unsigned mask = __ballot_sync(0xffffffffu, interior);
+        if (v) {
+            Real<L> oP = from_double<L>(0.0), oPi = from_double<L>(0.0);
+            if (interior) {
+                int rm = j - 1, rp = j + 1;
+                double sm = 1.0, sp = 1.0;
+                if (rm < 0) { rm = 0; sm = P.sigma; }
+                if (rp >= nt) { rp = nt - 1; sp = P.sigma; }
+                Real<L> bP = ut.get(cP, j, tc + 1), bPi = ut.get(cPi, j, tc + 1);
+                Real<L> cjv = Ld<L>::g(P.cj, nt, j);
+                substep_pair<L>(ht, p, sx, mask, j, rm, rp, sm, sp, tc, tc + 1, P.coef_i, P.plane, (long)j * P.pitch + i, cjv,
+                                P.tq_full, false, bP, bPi, oP, oPi);
+            }
+            const long g = (long)j * P.pitch + i;
+            Ld<L>::st(P.u_out + (long)cP * L * P.plane, P.plane, g, oP);
+            Ld<L>::st(P.u_out + (long)cPi * L * P.plane, P.plane, g, oPi);
+            if (P.obs_raw != nullptr) {
+                int di = i - P.oi, dj = j - P.oj;
+                if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
+                    long k = *P.step_base + P.step_off;
+                    if (k < P.obs_cap) {
+                        double* o = P.obs_raw + ((k * 4 + (dj * 2 + di)) * 4) * L;
+#pragma unroll
+                        for (int l = 0; l < L; ++l) { o[cP * L + l] = oP.x[l]; o[cPi * L + l] = oPi.x[l]; }
+                    }
+                }
+            }
+        }
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
 // Column kernel for the 10th-order theta operator (NEXT-1): a block owns TI radial columns and ALL
 // N_theta rows, so the +-5-row reach of each sub-step needs no theta halo (ghost rows are mirrored reads) and the
 // only redundant work is the one extra half-step column per block, (TI+1)/TI.  Same fusion as step_kernel.

@@ -420,7 +420,7 @@ extern "C" int teuk_set_option(teuk_ctx* c, const char* key, double value) {
         if (v == 0 ? !c->has_planes : !c->has_rc) return TEUK_EINVAL;      // that supply is not resident in this handle's workspace
         c->opt_cv = v;
     } else if (!strcmp(key, "variant")) {
-        if (v < 0 || v > 2) return TEUK_EINVAL;
+        if (v < 0 || v > 4) return TEUK_EINVAL;
         c->variant = v;
     } else if (!strcmp(key, "time_block")) {
         if ((v != 1 && v != 2) || (v == 2 && c->L != 1)) return TEUK_EINVAL;
@@ -696,14 +696,20 @@ static int choose_geometry(teuk_ctx* c) {
     }
     if (c->opt_tb == 2) return TEUK_EINVAL;        // time blocking exists only on the fp64 TMA stored-plane path
     int ti = c->opt_ti, tj = c->opt_tj;
+    // qd default: the pair kernel on its compile-time 16 x 16 tile (ragged edges are masked in the kernel, no clamping)
+    const bool qd_pair = c->L == 4 && (c->variant == 0 || c->variant == 3) && ti == 0 && tj == 0 && c->n_theta >= 12;
     if (ti == 0) ti = (c->L == 4) ? 16 : 32;
-    if (tj == 0) {
-        // whole theta extent when it fits (no theta halo, no redundant half-step rows), else strips of 16
-        int full = c->n_theta;
-        tj = (smem_bytes(c->L, ti, full) <= 100 * 1024 && full <= 64) ? full : ((c->L == 4) ? 8 : 16);
+    if (qd_pair) {
+        tj = 16;
+    } else {
+        if (tj == 0) {
+            // whole theta extent when it fits (no theta halo, no redundant half-step rows), else strips of 16
+            int full = c->n_theta;
+            tj = (smem_bytes(c->L, ti, full) <= 100 * 1024 && full <= 64) ? full : ((c->L == 4) ? 8 : 16);
+        }
+        if (tj > c->n_theta) tj = c->n_theta;
+        if (ti > c->n_r) ti = c->n_r;
     }
-    if (tj > c->n_theta) tj = c->n_theta;
-    if (ti > c->n_r) ti = c->n_r;
     size_t sm = smem_bytes(c->L, ti, tj);
     if (sm > 227 * 1024) return TEUK_EINVAL;
     c->ti = ti; c->tj = tj; c->smem = sm;

@@ -43,7 +43,9 @@ def main() -> int:
         ("full recompute, TMA tiles (step_kernel_f64_rc<full>)", 1, {"coef_variant": 2}),
         ("two iterations per launch (step2_kernel_f64_tma)", 1, {"time_block": 2}),
         ("double-double (step_kernel<2>)", 2, {}),
-        ("quad-double (step_kernel<4>)", 4, {}),
+        ("double-double, two threads per point (step_kernel_pair<2>)", 2, {"variant": 3, "tile_i": 32, "tile_j": 16}),
+        ("quad-double, two threads per point (step_kernel_pair<4>)", 4, {}),
+        ("quad-double, one thread per point (step_kernel<4>)", 4, {"variant": 4}),
         ("theta order 10, fp64 TMA columns, row runs (step_kernel_f64_col_run)", 1, {"theta_order": 10}),
         ("theta order 10, fp64 TMA columns, point per thread (step_kernel_f64_col_tma)", 1, {"theta_order": 10, "col_run": 0}),
         ("theta order 10, fp64 generic columns (step_kernel_col<1>)", 1, {"theta_order": 10, "use_tma": 0}),
@@ -70,6 +72,14 @@ def main() -> int:
                     note = f"  vs first fp64 family: {d:.1e}"
                 else:
                     ref[order] = u
+            elif order == 2:
+                # the dd / qd kernels of one precision perform the same operations in the same order: bitwise equal
+                if (L, order) in ref:
+                    same = bool(np.array_equal(u, ref[(L, order)]))
+                    fine = fine and same
+                    note = f"  bitwise == first {'dd' if L == 2 else 'qd'} family: {same}"
+                else:
+                    ref[(L, order)] = u
             print(f"m={m}  {'ok  ' if fine else 'FAIL'} {name}  tile {geom['tile_i']}x{geom['tile_j']}{note}", flush=True)
             ok = ok and fine
     # the allocation-free hook and the device build of the arithmetic layer

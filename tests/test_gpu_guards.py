@@ -19,7 +19,11 @@ FAMILIES = [
     ("f64_rc_full", 1, {"coef_variant": 2}),
     ("f64_tb2", 1, {"time_block": 2}),
     ("dd", 2, {}),
+    ("dd_pair", 2, {"variant": 3, "tile_i": 32, "tile_j": 16}),
     ("qd", 4, {}),
+    ("qd_pair_32x8", 4, {"variant": 3, "tile_i": 32, "tile_j": 8}),
+    ("qd_pair_16x8", 4, {"variant": 3, "tile_i": 16, "tile_j": 8}),
+    ("qd_one_thread_per_point", 4, {"variant": 4}),
     ("f64_col_run", 1, {"theta_order": 10}),
     ("f64_col_run8", 1, {"theta_order": 10, "tile_i": 8}),
     ("f64_col_tma", 1, {"theta_order": 10, "col_run": 0}),
@@ -64,6 +68,23 @@ def test_guard_bands_and_reproducibility(teuk, name, L, opts, n_r, n_theta, m):
     assert np.isfinite(u1).all() and np.isfinite(s1).all() and np.abs(u1[0, 0]).max() > 0
     assert np.array_equal(u1, u2) and np.array_equal(s1, s2), "run-to-run difference"
     assert np.all(u1[:, :, :, 0] == 0.0) and np.all(u1[:, :, :, -1] == 0.0)      # radial Dirichlet rows
+
+
+@pytest.mark.parametrize("L", [2, 4])
+@pytest.mark.parametrize("n_r,n_theta,m", [(131, 22, 2), (67, 12, 1), (40, 37, 2)])
+def test_pair_kernel_is_bitwise_the_one_thread_per_point_kernel(teuk, L, n_r, n_theta, m):
+    """step_kernel_pair (two lanes per point, partner values by shuffle) performs step_kernel's operations in
+    step_kernel's order: same bits in state and observer series, on ragged grids, for every pair tile shape"""
+    steps = 9
+    ref_opts = {"variant": 4} if L == 4 else {}
+    ref, sref, ok = _run(teuk, L, ref_opts, n_r, n_theta, m, steps)
+    assert ok
+    shapes = ([{}, {"variant": 3, "tile_i": 32, "tile_j": 8}, {"variant": 3, "tile_i": 16, "tile_j": 8}] if L == 4
+              else [{"variant": 3, "tile_i": 32, "tile_j": 16}])
+    for opts in shapes:
+        u, s, ok = _run(teuk, L, opts, n_r, n_theta, m, steps)
+        assert ok
+        assert np.array_equal(u, ref) and np.array_equal(s, sref), opts
 
 
 def test_march_kernel_is_independent_of_its_work_decomposition(teuk):
