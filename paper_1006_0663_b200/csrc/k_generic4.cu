@@ -23,7 +23,8 @@ const void* generic_step_fn_4(int variant, int ti, int tj, int* threads) {
     if (variant == 4 && ti == 16 && tj == 8) return (const void*)step_kernel<4, 16, 8, 128, 3>;
     return (const void*)step_kernel<4, 0, 0, 128, 3>;
 }
-const void* generic_col_fn_4(int* threads) {
+const void* generic_col_fn_4(int variant, int* threads) {
+    if (variant != 4) { *threads = 256; return (const void*)step_kernel_col_pair<4, 256, 2>; }
     *threads = 128;
     return (const void*)step_kernel_col<4, 128, 3>;
 }

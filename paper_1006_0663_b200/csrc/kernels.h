@@ -13,7 +13,7 @@ const void* generic_step_fn_4(int variant, int ti, int tj, int* threads);
 // step_kernel_col<L, THREADS, MINB> (10th-order theta operator)
 const void* generic_col_fn_1(int* threads);
 const void* generic_col_fn_2(int* threads);
-const void* generic_col_fn_4(int* threads);
+const void* generic_col_fn_4(int variant, int* threads);   // variant 4: one thread per point; else step_kernel_col_pair
 // fp64 TMA kernels (step_kernel_tma.cuh): stored planes, semi-recompute, 10th-order column kernel
 const void* tma_step_fn(int ti, int tj);
 const void* rc_step_fn(int ti, int tj, int full);     // full = H1b variant (c)

@@ -376,6 +376,24 @@ template <int L> __device__ __forceinline__ Real<L> partner(const Real<L>& a, un
     return r;
 }
 
+// tau * S_Pi and the two outputs of part p, in substep_core's order; sx = -1 (real part) / +1 (imaginary part) on the
+// cross terms
+template <int L>
+__device__ __forceinline__ void pair_tail(const GlobalCoef<L>& g, double sx, const Real<L>& sgP, const Real<L>& sgQ,
+                                          const Real<L>& sgPi, const Real<L>& sgQi, const Real<L>& dlP, const Real<L>& dlQ,
+                                          const Real<L>& dlPi, const Real<L>& lam, double tq, bool half, const Real<L>& baseP,
+                                          const Real<L>& basePi, Real<L>& outP, Real<L>& outPi) {
+    Real<L> s = neg(add(mul(g.get(1), sgPi), sgn(mul(g.get(2), sgQi), sx)));
+    s = add(s, add(mul(g.get(3), dlP), sgn(mul(g.get(4), dlQ), sx)));
+    s = add(s, mul(g.get(7), lam));
+    s = sub(s, add(mul(g.get(5), sgP), sgn(mul(g.get(6), sgQ), sx)));
+    const Real<L> c0 = g.get(0);
+    const Real<L> bP = half ? scale2(sgP, 0.5) : baseP;
+    const Real<L> bPi = half ? scale2(sgPi, 0.5) : basePi;
+    outP = add(sub(bP, mul(c0, dlP)), mul_d(sgPi, tq));
+    outPi = add(add(bPi, mul(c0, dlPi)), s);
+}
+
 // one sub-step for part p of one point; t: tile accessor; cf/stride/idx: the point's 8 folded coefficients in global memory
 template <int L, class Tile>
 __device__ __forceinline__ void substep_pair(const Tile& t, int p, double sx, unsigned mask, int row, int rm, int rp, double sm,
@@ -395,16 +413,46 @@ __device__ __forceinline__ void substep_pair(const Tile& t, int p, double sx, un
     const Real<L> second = sub(add(up, dn), scale2(sgP, 2.0));
     const Real<L> first = mul(cjv, sub(up, dn));
     const Real<L> lam = add(second, first);
-    // tau * S_Pi for this part, in substep_core's order; sx = -1 (real part) / +1 (imaginary part) on the cross terms
-    Real<L> s = neg(add(mul(g.get(1), sgPi), sgn(mul(g.get(2), sgQi), sx)));
-    s = add(s, add(mul(g.get(3), dlP), sgn(mul(g.get(4), dlQ), sx)));
-    s = add(s, mul(g.get(7), lam));
-    s = sub(s, add(mul(g.get(5), sgP), sgn(mul(g.get(6), sgQ), sx)));
-    const Real<L> c0 = g.get(0);
-    const Real<L> bP = half ? scale2(sgP, 0.5) : baseP;
-    const Real<L> bPi = half ? scale2(sgPi, 0.5) : basePi;
-    outP = add(sub(bP, mul(c0, dlP)), mul_d(sgPi, tq));
-    outPi = add(add(bPi, mul(c0, dlPi)), s);
+    pair_tail<L>(g, sx, sgP, sgQ, sgPi, sgQi, dlP, dlQ, dlPi, lam, tq, half, baseP, basePi, outP, outPi);
+}
+
+// stencil half-width 5 (substep_wide) for part p of one point; st: staged sig_Phi tile (both components, so the other
+// part's sig_Phi is a shared-memory read, not a shuffle)
+template <int L, class Tile, class STile>
+__device__ __forceinline__ void substep_wide_pair(const Tile& t, const STile& st, int scol, int p, double sx, unsigned mask, int row,
+                                                  int nt, double sigma, int clo, int chi, const double* __restrict__ cf,
+                                                  long stride, long idx, const Real<L>& cjv, const ThetaWeights& W, double tq,
+                                                  bool half, const Real<L>& baseP, const Real<L>& basePi, Real<L>& outP,
+                                                  Real<L>& outPi) {
+    const int cP = p, cPi = 2 + p;
+    GlobalCoef<L> g{cf, stride, idx};
+    const Real<L> sgP = st.get(cP, row, scol), sgQ = st.get(1 - p, row, scol);
+    Real<L> lo = t.get(cP, row, clo), hi = t.get(cP, row, chi);
+    const Real<L> dlP = sub(hi, lo);
+    lo = t.get(cPi, row, clo); hi = t.get(cPi, row, chi);
+    const Real<L> sgPi = add(hi, lo), dlPi = sub(hi, lo);
+    const Real<L> dlQ = partner(dlP, mask), sgQi = partner(sgPi, mask);
+    Real<L> w0;
+#pragma unroll
+    for (int l = 0; l < L; ++l) w0.x[l] = W.wd[0][l];
+    Real<L> s2 = mul(w0, sgP);
+    Real<L> s1 = from_double<L>(0.0);
+#pragma unroll 1
+    for (int k = 1; k <= 5; ++k) {
+        int ru = row + k, rd = row - k;
+        double su = 1.0, sd = 1.0;
+        if (ru >= nt) { ru = 2 * nt - 1 - ru; su = sigma; }
+        if (rd < 0) { rd = -rd - 1; sd = sigma; }
+        Real<L> up = sgn(st.get(cP, ru, scol), su);
+        Real<L> dn = sgn(st.get(cP, rd, scol), sd);
+        Real<L> wd, wc;
+#pragma unroll
+        for (int l = 0; l < L; ++l) { wd.x[l] = W.wd[k][l]; wc.x[l] = W.wc[k - 1][l]; }
+        s2 = add(s2, mul(wd, add(up, dn)));
+        s1 = add(s1, mul(wc, sub(up, dn)));
+    }
+    const Real<L> lam = add(s2, mul(cjv, scale2(s1, 2.0)));
+    pair_tail<L>(g, sx, sgP, sgQ, sgPi, sgQi, dlP, dlQ, dlPi, lam, tq, half, baseP, basePi, outP, outPi);
 }
 
 template <int L, int TI, int TJ, int NTHR, int MINB>
@@ -602,6 +650,107 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel_col(StepParams P, Thet
                     for (int c = 0; c < 4; ++c)
 #pragma unroll
                         for (int l = 0; l < L; ++l) o[c * L + l] = out[c].x[l];
+                }
+            }
+        }
+    }
+}
+
+// Pair version of step_kernel_col (same layout, same staging of sig_Phi): two lanes per point as in step_kernel_pair.
+template <int L, int NTHR, int MINB>
+__global__ void __launch_bounds__(NTHR, MINB) step_kernel_col_pair(StepParams P, ThetaWeights W) {
+    static_assert(NTHR % 64 == 0, "two lanes per point, whole warps");
+    extern __shared__ double smem[];
+    constexpr int NP = NTHR / 2;
+    const int TI = P.ti, nt = P.n_theta, nr = P.n_r;
+    const int UC = TI + 2, HC = TI + 1;
+    double* us = smem;                       // [4L][nt][UC]
+    double* hs = smem + 4 * L * nt * UC;     // [4L][nt][HC]
+    double* ss = hs + 4 * L * nt * HC;       // [2L][nt][HC]
+    const int i0 = blockIdx.x * TI, iu0 = i0 - 1;
+    const int tid = threadIdx.x;
+    const int p = tid & 1, cP = p, cPi = 2 + p;
+    const double sx = p ? 1.0 : -1.0;
+
+    const int n_stage = 4 * L * nt * UC;
+    for (int k = tid; k < n_stage; k += NTHR) {
+        int c = k % UC, rest = k / UC;
+        int r = rest % nt, pl = rest / nt;
+        int ui = iu0 + c;
+        bool ok = ui >= 0 && ui < nr;
+        cp_async8(us + k, ok ? P.u_in + pl * P.plane + (long)r * P.pitch + ui : P.u_in, ok);
+    }
+    cp_async_commit();
+    cp_async_wait<0>();
+    __syncthreads();
+
+    SmemTile<L> ut{us, nt, UC, 0};
+    for (int idx = tid; idx < 2 * nt * HC; idx += NTHR) {
+        int tc = idx % HC, rest = idx / HC;
+        int tr = rest % nt, c = rest / nt;
+        Real<L> sgm = add(ut.get(c, tr, tc + 1), ut.get(c, tr, tc));
+#pragma unroll
+        for (int l = 0; l < L; ++l) ss[(c * L + l) * nt * HC + tr * HC + tc] = sgm.x[l];
+    }
+    __syncthreads();
+    SmemTile<L> st1{ss, nt, HC, 0};
+    for (int q0 = 0; q0 < nt * HC; q0 += NP) {
+        const int q = q0 + (tid >> 1);
+        const int tr = q / HC, tc = q - tr * HC;
+        const int ih = iu0 + tc;
+        const bool v = q < nt * HC && ih >= 0 && ih <= nr - 2;
+        const unsigned mask = __ballot_sync(0xffffffffu, v);
+        if (v) {
+            Real<L> cjv = Ld<L>::g(P.cj, nt, tr);
+            Real<L> oP, oPi;
+            substep_wide_pair<L>(ut, st1, tc, p, sx, mask, tr, nt, P.sigma, tc, tc + 1, P.coef_h, P.plane, (long)tr * P.pitch + ih,
+                                 cjv, W, P.tq_half, true, oP, oPi, oP, oPi);
+#pragma unroll
+            for (int l = 0; l < L; ++l) {
+                hs[(cP * L + l) * nt * HC + tr * HC + tc] = oP.x[l];
+                hs[(cPi * L + l) * nt * HC + tr * HC + tc] = oPi.x[l];
+            }
+        }
+    }
+    __syncthreads();
+
+    SmemTile<L> ht{hs, nt, HC, 0};
+    for (int idx = tid; idx < 2 * nt * TI; idx += NTHR) {
+        int tc = idx % TI, rest = idx / TI;
+        int tr = rest % nt, c = rest / nt;
+        Real<L> sgm = add(ht.get(c, tr, tc + 1), ht.get(c, tr, tc));
+#pragma unroll
+        for (int l = 0; l < L; ++l) ss[(c * L + l) * nt * TI + tr * TI + tc] = sgm.x[l];
+    }
+    __syncthreads();
+    SmemTile<L> st2{ss, nt, TI, 0};
+    for (int q0 = 0; q0 < nt * TI; q0 += NP) {
+        const int q = q0 + (tid >> 1);
+        const int tr = q / TI, tc = q - tr * TI;
+        const int i = i0 + tc, j = tr;
+        const bool v = q < nt * TI && i < nr;
+        const bool interior = v && i != 0 && i != nr - 1;
+        const unsigned mask = __ballot_sync(0xffffffffu, interior);
+        if (v) {
+            Real<L> oP = from_double<L>(0.0), oPi = from_double<L>(0.0);
+            if (interior) {
+                Real<L> bP = ut.get(cP, j, tc + 1), bPi = ut.get(cPi, j, tc + 1);
+                Real<L> cjv = Ld<L>::g(P.cj, nt, j);
+                substep_wide_pair<L>(ht, st2, tc, p, sx, mask, j, nt, P.sigma, tc, tc + 1, P.coef_i, P.plane, (long)j * P.pitch + i,
+                                     cjv, W, P.tq_full, false, bP, bPi, oP, oPi);
+            }
+            const long g = (long)j * P.pitch + i;
+            Ld<L>::st(P.u_out + (long)cP * L * P.plane, P.plane, g, oP);
+            Ld<L>::st(P.u_out + (long)cPi * L * P.plane, P.plane, g, oPi);
+            if (P.obs_raw != nullptr) {
+                int di = i - P.oi, dj = j - P.oj;
+                if ((di == 0 || di == 1) && (dj == 0 || dj == 1)) {
+                    long k = *P.step_base + P.step_off;
+                    if (k < P.obs_cap) {
+                        double* o = P.obs_raw + ((k * 4 + (dj * 2 + di)) * 4) * L;
+#pragma unroll
+                        for (int l = 0; l < L; ++l) { o[cP * L + l] = oP.x[l]; o[cPi * L + l] = oPi.x[l]; }
+                    }
                 }
             }
         }

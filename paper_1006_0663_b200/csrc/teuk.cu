@@ -566,7 +566,7 @@ template <int TI> static bool setup_col_tma(teuk_ctx* c, bool row_run) {
 static const void* col_fn(const teuk_ctx* c, int* threads) {
     if (c->L == 1) return generic_col_fn_1(threads);
     if (c->L == 2) return generic_col_fn_2(threads);
-    return generic_col_fn_4(threads);
+    return generic_col_fn_4(c->variant, threads);
 }
 
 // centred 11-point weights from the textbook closed form c_k = (-1)^(k+1) (N!)^2 / (k (N-k)! (N+k)!), d_k = 2 c_k / k
@@ -626,6 +626,17 @@ static int choose_geometry(teuk_ctx* c) {
             if (ti > 32) ti = 32;
             if (c->L == 1 && ti >= 8) ti = (ti >= 16) ? 16 : 8;      // fp64: whole 64/128-byte rows per tile (measured best)
             if (ti < 2) ti = 2;
+            if (c->L == 4 && c->variant != 4) {
+                // pair kernel: 2 blocks/SM (110 KB each) of 256 threads = 128 points per pass over the sub-step code; among
+                // the tiles that fit take the one with the fewest passes per column (half step: (ti + 1) columns, full: ti)
+                const int tmax = std::max(2, std::min(32, (int)((110 * 1024 / per_col - 3.5) / 2.5)));
+                double best = 1e30;
+                for (int t = 2; t <= tmax; ++t) {
+                    const long nt = c->n_theta;
+                    const double cost = (double)(((t + 1) * nt + 127) / 128 + (t * nt + 127) / 128) / t;
+                    if (cost <= best) { best = cost; ti = t; }
+                }
+            }
         }
         if (ti > c->n_r) ti = c->n_r;
         size_t sm = (size_t)4 * c->L * 8 * c->n_theta * (2 * ti + 3) + (size_t)2 * c->L * 8 * c->n_theta * (ti + 1);
