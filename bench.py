@@ -310,13 +310,15 @@ def kernel_name(L, options):
     if "theta_order=10" in opt:
         if L == 1:
             return "step_kernel_col<1>" if "use_tma=0" in opt else ("step_kernel_f64_col_tma" if "col_run=0" in opt else "step_kernel_f64_col_run")
-        return f"step_kernel_col<{L}>"
+        return "step_kernel_col_pair<4>" if (L == 4 and "variant=4" not in opt) else f"step_kernel_col<{L}>"
     if L == 1:
         if "coef_variant=1" in opt:
             return "step_kernel_f64_rc" if "march=0" in opt else "step_kernel_f64_march"
         if "coef_variant=2" in opt:
             return "step_kernel_f64_rc<full>"
         return "step2_kernel_f64_tma" if "time_block=2" in opt else "step_kernel_f64_tma"
+    if L == 4 and "variant=4" not in opt:
+        return "step_kernel_pair<4>"
     return f"step_kernel<{L}>"
 
 
