@@ -563,25 +563,17 @@ __global__ void __launch_bounds__(MAXT, MINB) step_kernel_col(StepParams P, Thet
     const int i0 = blockIdx.x * TI, iu0 = i0 - 1;
     const int tid = threadIdx.x, nth = MAXT;
 
-    // stage the u^n columns; loads in batches of STG before any store (one memory round trip per batch)
-    constexpr int STG = 8;
+    // stage the u^n columns (8-byte zero-fill cp.async: the whole tile in flight at once, as in step_kernel)
     const int n_stage = 4 * L * nt * UC;
-    for (int k0 = tid; k0 < n_stage; k0 += nth * STG) {
-        double vals[STG];
-#pragma unroll
-        for (int u = 0; u < STG; ++u) {
-            int k = k0 + u * nth;
-            int c = k % UC, rest = k / UC;
-            int r = rest % nt, pl = rest / nt;
-            int ui = iu0 + c;
-            vals[u] = (k < n_stage && ui >= 0 && ui < nr) ? __ldg(P.u_in + pl * P.plane + (long)r * P.pitch + ui) : 0.0;
-        }
-#pragma unroll
-        for (int u = 0; u < STG; ++u) {
-            int k = k0 + u * nth;
-            if (k < n_stage) us[k] = vals[u];
-        }
+    for (int k = tid; k < n_stage; k += nth) {
+        int c = k % UC, rest = k / UC;
+        int r = rest % nt, pl = rest / nt;
+        int ui = iu0 + c;
+        bool ok = ui >= 0 && ui < nr;
+        cp_async8(us + k, ok ? P.u_in + pl * P.plane + (long)r * P.pitch + ui : P.u_in, ok);
     }
+    cp_async_commit();
+    cp_async_wait<0>();
     __syncthreads();
 
     SmemTile<L> ut{us, nt, UC, 0};

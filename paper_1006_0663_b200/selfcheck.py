@@ -50,7 +50,8 @@ def main() -> int:
         ("theta order 10, fp64 TMA columns, point per thread (step_kernel_f64_col_tma)", 1, {"theta_order": 10, "col_run": 0}),
         ("theta order 10, fp64 generic columns (step_kernel_col<1>)", 1, {"theta_order": 10, "use_tma": 0}),
         ("theta order 10, double-double (step_kernel_col<2>)", 2, {"theta_order": 10}),
-        ("theta order 10, quad-double (step_kernel_col<4>)", 4, {"theta_order": 10}),
+        ("theta order 10, quad-double, two threads per point (step_kernel_col_pair<4>)", 4, {"theta_order": 10}),
+        ("theta order 10, quad-double, one thread per point (step_kernel_col<4>)", 4, {"theta_order": 10, "variant": 4}),
     ]
     for m in (2, 1):                                      # even and odd |m| (polar ghost sign)
         ref = {}
@@ -72,8 +73,8 @@ def main() -> int:
                     note = f"  vs first fp64 family: {d:.1e}"
                 else:
                     ref[order] = u
-            elif order == 2:
-                # the dd / qd kernels of one precision perform the same operations in the same order: bitwise equal
+            else:
+                # the dd / qd kernels of one precision and theta order perform the same operations in the same order: bitwise equal
                 if (L, order) in ref:
                     same = bool(np.array_equal(u, ref[(L, order)]))
                     fine = fine and same

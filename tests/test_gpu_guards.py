@@ -30,6 +30,7 @@ FAMILIES = [
     ("f64_col", 1, {"theta_order": 10, "use_tma": 0}),
     ("dd_col", 2, {"theta_order": 10}),
     ("qd_col", 4, {"theta_order": 10}),
+    ("qd_col_one_thread_per_point", 4, {"theta_order": 10, "variant": 4}),
 ]
 
 
@@ -85,6 +86,12 @@ def test_pair_kernel_is_bitwise_the_one_thread_per_point_kernel(teuk, L, n_r, n_
         u, s, ok = _run(teuk, L, opts, n_r, n_theta, m, steps)
         assert ok
         assert np.array_equal(u, ref) and np.array_equal(s, sref), opts
+    if L == 4:      # theta order 10: step_kernel_col_pair against step_kernel_col
+        ref, sref, ok = _run(teuk, 4, {"theta_order": 10, "variant": 4}, n_r, n_theta, m, steps)
+        for opts in ({"theta_order": 10}, {"theta_order": 10, "tile_i": 3}, {"theta_order": 10, "tile_i": 8}):
+            u, s, ok2 = _run(teuk, 4, opts, n_r, n_theta, m, steps)
+            assert ok and ok2
+            assert np.array_equal(u, ref) and np.array_equal(s, sref), opts
 
 
 def test_march_kernel_is_independent_of_its_work_decomposition(teuk):
