@@ -86,7 +86,9 @@ int teuk_create_slab(double M, double a, int s, int m, int n_r_global, int n_the
  *                  kernel, two threads per point, 16 x 16 tile); 1, 2 = one thread per point with other launch bounds;
  *                  3 = pair kernel (dd 32 x 16; qd 16 x 16, 32 x 8 or 16 x 8 by tile_i / tile_j); 4 = qd one thread per
  *                  point on its 16 x 8 tile (the default before the pair kernel).  All bitwise identical in result.
- *  "pdl"           fp64 TMA kernels: 1 = programmatic dependent launch (default 0; measured neutral).
+ *  "pdl"           programmatic dependent launch of the step kernel (the next step's blocks start their set-up while this
+ *                  step drains; results are bitwise the same): 1 = on, 0 = off.  Default: on for the fp64 column-march kernel
+ *                  (+2.7 % on config 2), off for the fp64 TMA kernels (measured neutral); other kernels ignore it.
  *  "time_block"    1 = one iteration per launch (default); 2 = EXPERIMENT: two iterations per launch on a shared-memory
  *                  resident tile, fp64 stored-plane TMA path only, else TEUK_EINVAL at teuk_set_initial; an odd last
  *                  iteration and runs with the multipole observer use the one-iteration kernel.  Parity-green but slower

@@ -81,6 +81,9 @@ constexpr size_t march_smem_bytes(int n_theta) {
 template <int MINB>                  // blocks per SM the register budget is cut for
 __global__ void __launch_bounds__(32 * MARCH_WARPS, MINB) step_kernel_f64_march(StepParams P, MarchParams Q) {
     extern __shared__ double sm[];
+    // programmatic dependent launch ("pdl" option): the next step's blocks may be scheduled as this step's blocks exit and
+    // run their set-up (theta tables, ring clearing, r-table registers); they wait below before touching the state
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const int nt = P.n_theta, nr = P.n_r;
     double* tht = sm;                                                // [4][nt]: cj, sin^2, cos, Tth
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -137,6 +140,7 @@ __global__ void __launch_bounds__(32 * MARCH_WARPS, MINB) step_kernel_f64_march(
             cp_async8(dst + 5 * 32, Q.isig_i + (row + (unsigned)cic), inr && c_ok);
             cp_async_commit();
         };
+        asm volatile("griddepcontrol.wait;" ::: "memory");          // u^n (written by the previous step) is complete and visible
 #pragma unroll 1
         for (int r = ua; r < ua + MARCH_PF; ++r) request(r);
 

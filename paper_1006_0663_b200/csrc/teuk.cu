@@ -92,7 +92,7 @@ struct teuk_ctx {
     cudaStream_t stream;
     SetupConsts C;
     // options
-    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0, theta_order = 2, opt_pdl = 0, opt_tb = 1;   // PDL measured neutral on cfg 2 (40.2 vs 40.0 us): kept as an option
+    int graph_steps = 32, opt_ti = 0, opt_tj = 0, opt_tma = 1, variant = 0, coef_variant = 0, theta_order = 2, opt_pdl = -1, opt_tb = 1;   // PDL measured neutral on cfg 2 (40.2 vs 40.0 us): kept as an option
     ThetaWeights tw;
     // TMA path (fp64): tensor maps of the two state buffers and the two coefficient families
     bool use_tma = false, use_rc = false, use_col_tma = false, use_march = false;
@@ -767,8 +767,14 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         Q.chunk_rows = c->march_chunk;
         Q.n_units = c->march_units;
         void* args[] = {&P, &Q};
-        if (cudaLaunchKernel(march_step_fn(), c->grid, dim3(c->threads), args, c->smem, c->stream) != cudaSuccess)
-            return TEUK_ECUDA;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = c->grid; cfg.blockDim = dim3(c->threads); cfg.dynamicSmemBytes = c->smem; cfg.stream = c->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = c->opt_pdl != 0 ? 1 : 0;      // automatic (-1) = on: +2.7 % on cfg 2, +1.6 % on 65536 x 64
+        cudaError_t le = cudaLaunchKernelExC(&cfg, march_step_fn(), args);
+        if (le != cudaSuccess) return cuda_fail(le, "cudaLaunchKernelEx(march kernel)", __LINE__);
     } else if (c->use_rc || c->use_tma) {
         // programmatic dependent launch: the next step's blocks may start (and prefetch their coefficient tiles) while this
         // step drains; they execute griddepcontrol.wait before touching the state
@@ -777,7 +783,7 @@ static int launch_step(teuk_ctx* c, int from, int step_off) {
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = at; cfg.numAttrs = c->opt_pdl ? 1 : 0;
+        cfg.attrs = at; cfg.numAttrs = c->opt_pdl == 1 ? 1 : 0;
         cudaError_t le;
         RcParams Q{c->dptr(c->lay.rc_th)};
         if (c->use_rc) {
@@ -832,7 +838,7 @@ static int launch_step2(teuk_ctx* c, int from, int step_off) {
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = c->opt_pdl ? 1 : 0;
+    cfg.attrs = at; cfg.numAttrs = c->opt_pdl == 1 ? 1 : 0;
     void* args[] = {&c->tm2_state[from], &c->tm2_ch, &P};
     cudaError_t le = cudaLaunchKernelExC(&cfg, tb2_step_fn(c->ti, c->tj), args);
     if (le != cudaSuccess) return cuda_fail(le, "cudaLaunchKernelExC(step2 kernel)", __LINE__);

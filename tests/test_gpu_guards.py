@@ -96,10 +96,12 @@ def test_pair_kernel_is_bitwise_the_one_thread_per_point_kernel(teuk, L, n_r, n_
 
 def test_march_kernel_is_independent_of_its_work_decomposition(teuk):
     """the column-march kernel cut into work units of different lengths (and the tile kernel of the same supply) gives
-    the same bits: no dependence on which warp handled which rows, no stale ring slots between units"""
+    the same bits: no dependence on which warp handled which rows, no stale ring slots between units; nor on whether the
+    steps are launched programmatically dependent (default) or fully serialised ("pdl" = 0)"""
     ref = None
     for opts in ({"coef_variant": 1}, {"coef_variant": 1, "march_chunk": 5}, {"coef_variant": 1, "march_chunk": 8},
-                 {"coef_variant": 1, "march_chunk": 23}, {"coef_variant": 1, "march_chunk": 37}):
+                 {"coef_variant": 1, "march_chunk": 23}, {"coef_variant": 1, "march_chunk": 37},
+                 {"coef_variant": 1, "pdl": 0}, {"coef_variant": 1, "pdl": 0, "march_chunk": 8}):
         u, ser, ok = _run(teuk, 1, opts, 333, 37, 2, 33)
         assert ok
         if ref is None:
